@@ -1,0 +1,278 @@
+"""Pins of the CPU oracle (oracle/pca_oracle.cpp) against what the paper and the mathematics fix.
+
+Nothing here compares the oracle with itself or with the CUDA path: expected values are hand
+derivations (tests/golden/*.json, cited), closed forms, invariants the paper states (eq. 4,
+orthogonality, "full SVD for K = N"), library routines (numpy SVD / eigh / mean) and brute
+force (cyclic Jacobi on X^T X).  All run on CPU (`-m "not gpu"`).
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_0811_1081_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _abs_cos(a, b):
+    return abs(float(a @ b)) / (np.linalg.norm(a) * np.linalg.norm(b))
+
+
+# ----------------------------------------------------------------------------- worked examples
+def test_golden_worked_3x2_nipals(oracle_mod):
+    g = json.load(open(os.path.join(GOLD, "worked_3x2.json")))
+    X = np.array(g["X_rows"], dtype=np.float64)
+    r = oracle_mod.pca(X, g["K"], g["eps"], g["max_iter"], oracle_mod.ALGO_NIPALS)
+    assert list(r.iters) == g["iters"]
+    lam = math.sqrt(g["lambda_sq_num"] / g["lambda_sq_den"])
+    nrm = math.sqrt(g["norm_sq"])
+    assert abs(r.lam[0] - lam) <= 1e-14 * lam
+    np.testing.assert_allclose(r.P[:, 0], np.array(g["p_int"]) / nrm, rtol=1e-14, atol=0)
+    np.testing.assert_allclose(r.T[:, 0], np.array(g["t_int"]) / nrm, rtol=1e-14, atol=0)
+    R = X - np.outer(g["t_int"], g["p_int"]) / g["norm_sq"]          # eq. (3)
+    np.testing.assert_allclose(r.R, R, rtol=0, atol=1e-14)
+    # one pass only (max_iter = 1) returns the pass-1 lambda: pins "lambda' is taken every pass"
+    r1 = oracle_mod.pca(X, 1, 1.0, 1, oracle_mod.ALGO_NIPALS)
+    assert list(r1.iters) == [1]
+    lam1 = math.sqrt(g["lambda_pass1_sq_num"] / g["lambda_pass1_sq_den"])
+    assert abs(r1.lam[0] - lam1) <= 1e-14 * lam1
+
+
+@pytest.mark.parametrize("algo", [0, 1])
+def test_golden_diag_2x2(oracle_mod, algo):
+    g = json.load(open(os.path.join(GOLD, "diag_2x2.json")))
+    X = np.array(g["X_rows"], dtype=np.float64)
+    r = oracle_mod.pca(X, g["K"], g["eps"], g["max_iter"], algo)
+    assert list(r.iters) == g["iters"]
+    np.testing.assert_array_equal(r.lam, np.array(g["lambda"], dtype=np.float64))
+    np.testing.assert_array_equal(r.T, np.array(g["T_rows"], dtype=np.float64))
+    np.testing.assert_array_equal(r.P, np.array(g["P_rows"], dtype=np.float64))
+    np.testing.assert_array_equal(r.R, np.array(g["R_rows"], dtype=np.float64))
+
+
+# ----------------------------------------------------------------------------- P1 prescribed spectrum
+@pytest.mark.parametrize("algo", [0, 1])
+def test_prescribed_spectrum_noise_free(oracle_mod, algo):
+    """X = U diag(s) V^T exactly (no noise): lambda_k = s_k, P = +-V, T = +-s_k U."""
+    cfg = inputs.scaled(inputs.config(0), 256, 64, K=8, noise=0.0)
+    pr = inputs.generate(cfg, keep_factors=True)
+    # use the float64 product, not the float32 cast, so the pin is at double precision
+    U, V, s = pr.truth["U"], pr.truth["V"], pr.truth["s"]
+    X = oracle_mod.center((U * s[None, :]) @ V.T)
+    r = oracle_mod.pca(X, 8, 1e-14, 10000, algo)
+    assert np.all(r.iters < 10000) and np.all(r.iters >= 2)
+    np.testing.assert_allclose(r.lam, s[:8], rtol=1e-11)
+    for k in range(8):
+        assert _abs_cos(r.P[:, k], V[:, k]) >= 1 - 1e-11
+        assert _abs_cos(r.T[:, k], U[:, k]) >= 1 - 1e-11
+        assert abs(np.linalg.norm(r.T[:, k]) - r.lam[k]) <= 1e-12 * r.lam[k]
+        assert abs(np.linalg.norm(r.P[:, k]) - 1.0) <= 1e-14
+        # joint sign: T[:,k] P[:,k]^T is the rank-1 term s_k U_k V_k^T
+        sg = np.sign(r.P[:, k] @ V[:, k])
+        # lambda stagnates quadratically faster than the vector converges (Rayleigh quotient), so a
+        # 1e-14 stagnation test leaves an O(1e-7) angle: elementwise agreement is ~1e-7, not 1e-14
+        np.testing.assert_allclose(sg * r.T[:, k], s[k] * U[:, k], atol=2e-6)
+
+
+# ----------------------------------------------------------------------------- P2 Jacobi, P3 SVD
+def test_jacobi_matches_library_eigh(oracle_mod):
+    rng = np.random.default_rng(5)
+    A = rng.standard_normal((40, 40))
+    A = A + A.T
+    w, V, sweeps = oracle_mod.jacobi_eigh(A)
+    assert 1 <= sweeps < 60
+    wl = np.linalg.eigvalsh(A)
+    np.testing.assert_allclose(np.sort(w), wl, rtol=0, atol=1e-12 * np.abs(wl).max())
+    np.testing.assert_allclose(V.T @ V, np.eye(40), atol=1e-13)
+    np.testing.assert_allclose(A @ V, V * w[None, :], atol=1e-12 * np.abs(wl).max())
+
+
+@pytest.mark.parametrize("algo", [0, 1])
+def test_cfg1_against_jacobi_and_svd(oracle_mod, algo):
+    """Config 1: converged values are the eigen-pairs of X^T X (brute force) / the SVD (library)."""
+    cfg = inputs.config(0)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    r = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, algo)
+    w, Vec, _ = oracle_mod.jacobi_eigh(X.T @ X)
+    order = np.argsort(-w)
+    sv = np.linalg.svd(X, compute_uv=False)
+    for k in range(cfg.K):
+        # "maximum error eps for eigenvalues": eps = 1e-7 relative stagnation test
+        assert abs(r.lam[k] ** 2 / w[order[k]] - 1) <= 5e-6
+        assert abs(r.lam[k] / sv[k] - 1) <= 5e-6
+        assert _abs_cos(r.P[:, k], Vec[:, order[k]]) >= 1 - 1e-5
+
+
+def test_scaled_cfg2_against_svd(oracle_mod):
+    cfg = inputs.scaled(inputs.config(1), 512, 128, K=16)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    r = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, oracle_mod.ALGO_GS)
+    Us, sv, Vt = np.linalg.svd(X, full_matrices=False)
+    np.testing.assert_allclose(r.lam, sv[:cfg.K], rtol=5e-6)
+    for k in range(cfg.K):
+        assert _abs_cos(r.P[:, k], Vt[k]) >= 1 - 1e-4
+        assert _abs_cos(r.T[:, k], Us[:, k]) >= 1 - 1e-4
+
+
+def test_K1_is_top_singular_triplet(oracle_mod):
+    rng = np.random.default_rng(11)
+    X = oracle_mod.center(rng.standard_normal((200, 30)) * np.linspace(3, 1, 30)[None, :])
+    Us, sv, Vt = np.linalg.svd(X, full_matrices=False)
+    for algo in (0, 1):
+        r = oracle_mod.pca(X, 1, 1e-13, 100000, algo)
+        assert abs(r.lam[0] / sv[0] - 1) <= 1e-9
+        assert _abs_cos(r.P[:, 0], Vt[0]) >= 1 - 1e-9
+        assert _abs_cos(r.T[:, 0], Us[:, 0]) >= 1 - 1e-9
+
+
+# ----------------------------------------------------------------------------- P4, P5 identities
+@pytest.mark.parametrize("algo", [0, 1])
+@pytest.mark.parametrize("eps", [1e-3, 1e-9])
+def test_energy_and_decomposition_identities(oracle_mod, algo, eps):
+    """eq. (4) X = T_K P_K^T + R elementwise, and ||R||_F^2 = ||X||_F^2 - sum lambda_k^2, any eps."""
+    cfg = inputs.scaled(inputs.config(2), 300, 80, K=12)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    r = oracle_mod.pca(X, cfg.K, eps, 10000, algo)
+    np.testing.assert_allclose(r.T @ r.P.T + r.R, X, rtol=0, atol=1e-11 * np.abs(X).max())
+    e_x, e_r = np.sum(X * X), np.sum(r.R * r.R)
+    assert abs(e_x - np.sum(r.lam ** 2) - e_r) <= 1e-12 * e_x
+    for k in range(cfg.K):
+        assert abs(np.linalg.norm(r.T[:, k]) - r.lam[k]) <= 1e-12 * r.lam[k]
+
+
+# ----------------------------------------------------------------------------- P6 orthogonality
+def test_gs_orthogonality_and_nipals_loss(oracle_mod):
+    """GS-PCA: loads AND scores orthogonal; NIPALS scores are not."""
+    cfg = inputs.config(0)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    g = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, oracle_mod.ALGO_GS)
+    n = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, oracle_mod.ALGO_NIPALS)
+    I = np.eye(cfg.K)
+
+    def offdiag(T):
+        Vn = T / np.linalg.norm(T, axis=0, keepdims=True)
+        return np.max(np.abs(Vn.T @ Vn - I))
+
+    assert np.max(np.abs(g.P.T @ g.P - I)) <= 1e-12
+    assert offdiag(g.T) <= 1e-12
+    assert offdiag(n.T) > 1e-8          # early stopping leaves NIPALS scores visibly non-orthogonal
+    assert offdiag(n.T) > 1e3 * offdiag(g.T)
+
+
+def test_gs_orthogonality_collinear(oracle_mod):
+    cfg = inputs.scaled(inputs.config(2), 400, 96, K=24)        # X = A B + noise, rank-16 signal
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    g = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, oracle_mod.ALGO_GS)
+    I = np.eye(cfg.K)
+    Vn = g.T / g.lam[None, :]
+    assert np.max(np.abs(g.P.T @ g.P - I)) <= 1e-12
+    assert np.max(np.abs(Vn.T @ Vn - I)) <= 1e-12
+
+
+# ----------------------------------------------------------------------------- P7 K = N
+def test_full_decomposition_K_equals_N(oracle_mod):
+    """K = N: 'full SVD ... with a maximum error eps for eigenvalues'."""
+    cfg = inputs.scaled(inputs.config(4), 256, 32, K=32)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    r = oracle_mod.pca(X, 32, 1e-10, 100000, oracle_mod.ALGO_GS)
+    sv = np.linalg.svd(X, compute_uv=False)
+    np.testing.assert_allclose(np.sort(r.lam)[::-1], sv, rtol=1e-6)
+    assert np.linalg.norm(X - r.T @ r.P.T) <= 1e-3 * np.linalg.norm(X)
+    assert np.max(np.abs(r.P.T @ r.P - np.eye(32))) <= 1e-12
+    assert np.max(np.abs(r.P @ r.P.T - np.eye(32))) <= 1e-12      # square orthogonal
+
+
+# ----------------------------------------------------------------------------- P8 control flow
+def test_eps_zero_runs_exactly_max_iter(oracle_mod):
+    rng = np.random.default_rng(3)
+    X = rng.standard_normal((50, 10))
+    for algo in (0, 1):
+        r = oracle_mod.pca(X, 3, 0.0, 17, algo)       # strict '<' never fires with eps = 0
+        assert list(r.iters) == [17, 17, 17]
+
+
+def test_eps_one_stops_at_second_pass(oracle_mod):
+    """lambda starts at 0 and the test is strict: pass 1 cannot fire, pass 2 does."""
+    rng = np.random.default_rng(4)
+    X = rng.standard_normal((50, 10))
+    for algo in (0, 1):
+        r = oracle_mod.pca(X, 3, 1.0, 100, algo)
+        assert list(r.iters) == [2, 2, 2]
+
+
+def test_rank_one_converges_in_two_passes(oracle_mod):
+    rng = np.random.default_rng(6)
+    a, b = rng.standard_normal(64), rng.standard_normal(12)
+    X = np.outer(a, b)
+    for algo in (0, 1):
+        r = oracle_mod.pca(X, 1, 1e-12, 100, algo)
+        assert r.iters[0] == 2
+        assert abs(r.lam[0] - np.linalg.norm(a) * np.linalg.norm(b)) <= 1e-12 * r.lam[0]
+        assert _abs_cos(r.P[:, 0], b) >= 1 - 1e-14
+
+
+def test_gs_first_component_equals_nipals(oracle_mod):
+    """For k = 0 no projection is applied; GS-PCA only rescales t each pass."""
+    cfg = inputs.config(0)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    g = oracle_mod.pca(X, 1, cfg.eps, cfg.max_iter, oracle_mod.ALGO_GS)
+    n = oracle_mod.pca(X, 1, cfg.eps, cfg.max_iter, oracle_mod.ALGO_NIPALS)
+    assert g.iters[0] == n.iters[0]
+    assert abs(g.lam[0] - n.lam[0]) <= 1e-13 * n.lam[0]
+    np.testing.assert_allclose(g.P, n.P, atol=1e-13)
+    np.testing.assert_allclose(g.T, n.T, atol=1e-12)
+
+
+def test_degenerate_zero_column_and_zero_matrix(oracle_mod):
+    rng = np.random.default_rng(8)
+    X = rng.standard_normal((30, 6))
+    X[:, 1] = 0.0                                   # start column of component 1 is exactly zero
+    for algo in (0, 1):
+        r = oracle_mod.pca(X, 3, 1e-9, 1000, algo)
+        assert r.iters[1] == 0 and r.lam[1] == 0.0
+        assert not r.T[:, 1].any() and not r.P[:, 1].any()
+        assert r.iters[0] >= 2 and r.iters[2] >= 2
+        np.testing.assert_allclose(r.T @ r.P.T + r.R, X, atol=1e-12)
+        z = oracle_mod.pca(np.zeros((5, 3)), 2, 1e-7, 10, algo)
+        assert list(z.iters) == [0, 0] and not z.lam.any() and not z.R.any()
+
+
+def test_invalid_arguments(oracle_mod):
+    X = np.ones((4, 3))
+    for bad in (dict(K=0), dict(K=4), dict(eps=-1.0), dict(max_iter=0), dict(algo=2)):
+        kw = dict(K=2, eps=1e-7, max_iter=10, algo=0)
+        kw.update(bad)
+        with pytest.raises(ValueError):
+            oracle_mod.pca(X, **kw)
+
+
+# ----------------------------------------------------------------------------- centring
+def test_center_matches_library_mean(oracle_mod):
+    rng = np.random.default_rng(9)
+    X = rng.standard_normal((123, 17)) + 100.0 * rng.standard_normal(17)[None, :]
+    Xc = oracle_mod.center(X)
+    np.testing.assert_allclose(Xc, X - X.mean(axis=0, keepdims=True), atol=1e-12)
+    assert np.max(np.abs(Xc.sum(axis=0))) <= 1e-10
+    # literal eq. (1): the mean COLUMN is removed, so every ROW sums to zero and rank drops by one
+    Xe = oracle_mod.center_eq1(X)
+    np.testing.assert_allclose(Xe, X - X.mean(axis=1, keepdims=True), atol=1e-12)
+    assert np.linalg.matrix_rank(Xe) == 16
+
+
+# ----------------------------------------------------------------------------- determinism
+def test_thread_count_independence(oracle_mod):
+    cfg = inputs.scaled(inputs.config(1), 700, 96, K=6)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    n0 = oracle_mod.num_threads()
+    try:
+        oracle_mod.set_num_threads(1)
+        a = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, oracle_mod.ALGO_GS)
+        oracle_mod.set_num_threads(max(2, n0))
+        b = oracle_mod.pca(X, cfg.K, cfg.eps, cfg.max_iter, oracle_mod.ALGO_GS)
+    finally:
+        oracle_mod.set_num_threads(n0)
+    assert np.array_equal(a.iters, b.iters)
+    assert np.array_equal(a.lam, b.lam) and np.array_equal(a.T, b.T) and np.array_equal(a.P, b.P)

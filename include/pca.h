@@ -1,0 +1,148 @@
+/* =====================================================================================
+ * include/pca.h -- C ABI of the B200-native (sm_100a) hot path of Andrecut's iterative PCA
+ * (arxiv 0811.1081, "Parallel GPU Implementation of Iterative PCA Algorithms"; the paper text
+ * is cited as PAPER.md:<line>).
+ *
+ * The library computes, for a column-mean-centred M x N matrix X, the
+ * truncated decomposition X = T_(K) P_(K)^T + R (eq. 4) one component at a time
+ * with the power-style inner loop of NIPALS-PCA (section 2.2; listing
+ * PAPER.md:555-568) or GS-PCA (section 2.3; listing PAPER.md:1016-1038).
+ * Every step of that loop (loads p = R^T t, Gram-Schmidt against the previous loadings,
+ * normalisation, scores t = R p, Gram-Schmidt against the previous scores, lambda = ||t||,
+ * convergence test, rank-1 deflation) runs in hand-written CUDA kernels; the convergence test is
+ * taken on the device, so no call below reads device data back to the host.
+ *
+ * Conventions
+ *   layout     column-major, leading dimension = number of rows: element (m, n) of an M x N
+ *              matrix is at index n*M + m, the paper's id(m,n,ld).
+ *              A contiguous row-major (N, M) array IS the M x N column-major matrix.
+ *   precision  fp32 storage and fp32 FMA in the two big matrix-vector products; norms, Gram-
+ *              Schmidt coefficients, lambda and the convergence test are fp64 scalars on device.
+ *   pointers   "dev" = device memory of the current CUDA device, "host" = host memory.
+ *              Device matrices must be 16-byte aligned (PCA_EALIGN otherwise).
+ *   stream     a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   async      pca_center / pca_run only ENQUEUE work on `stream` and return; results are valid
+ *              once the caller has synchronised the stream.  Argument and launch errors are
+ *              returned synchronously.  Nothing prints, throws or exits.
+ *   ownership  the caller owns X, T, P, lambda, iters and the workspace; the context owns only
+ *              host memory (plus, if pca_fit_host is used, its private device staging buffers).
+ *   threads    one context = one problem shape; a context is not thread-safe; distinct
+ *              contexts on distinct streams are independent.
+ *   errors     every int-returning call returns PCA_OK (0) or one of the codes below.
+ * ===================================================================================== */
+#ifndef PCA_H_
+#define PCA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pca_ctx pca_ctx; /* opaque */
+
+enum { PCA_ALGO_NIPALS = 0, PCA_ALGO_GS = 1 };
+
+enum {
+  PCA_OK = 0,
+  PCA_EINVAL = 1,       /* bad argument (see each call) */
+  PCA_EALIGN = 2,       /* a device matrix pointer is not 16-byte aligned */
+  PCA_ECUDA = 3,        /* a CUDA runtime call failed (pca_last_cuda_error has the code) */
+  PCA_EWORKSPACE = 4,   /* no workspace set, or it is smaller than pca_workspace_bytes() */
+  PCA_EUNSUPPORTED = 5  /* shape cannot be handled by this build (e.g. N too large for SMEM) */
+};
+
+/* Options for pca_set_option (all optional; defaults are chosen by pca_create). */
+enum {
+  PCA_OPT_PATH = 1,     /* 0 = auto, 1 = force HBM-streaming path, 2 = force SMEM-resident path */
+  PCA_OPT_CTAS = 2,     /* number of CTAs of the persistent kernel (0 = auto) */
+  PCA_OPT_CENTER_MODE = 3 /* 0 = column means (default), 1 = literal eq. (1) mean column */
+};
+
+/* Fields for pca_get_info. */
+enum {
+  PCA_INFO_PATH = 1,        /* 1 = streaming, 2 = resident */
+  PCA_INFO_CTAS = 2,        /* CTAs of the persistent solve kernel */
+  PCA_INFO_THREADS = 3,     /* threads per CTA */
+  PCA_INFO_SMEM_BYTES = 4,  /* dynamic shared memory per CTA */
+  PCA_INFO_ROWS_PER_CTA = 5,
+  PCA_INFO_LAUNCHES_PER_RUN = 6, /* kernel launches one pca_run enqueues */
+  PCA_INFO_NUM_SMS = 7
+};
+
+/* Create a context for one problem shape.
+ *   M, N      rows (observations) and columns (attributes) of X, M >= 1, N >= 1
+ *   K         number of components, 1 <= K <= N ("K <= N"; the start vector of
+ *             component k is column k of the residual)
+ *   eps       >= 0; relative stagnation tolerance of the listings' test
+ *             |lambda - lambda'| < eps * lambda'.  eps = 0 never fires,
+ *             i.e. exactly max_iter passes per component (fixed-work benchmark mode)
+ *   max_iter  >= 1; the listings' J = 10000
+ *   algo      PCA_ALGO_NIPALS or PCA_ALGO_GS
+ * Needs a CUDA device (queries its SM count and shared-memory size); PCA_ECUDA if there is none.
+ * Errors: PCA_EINVAL, PCA_ECUDA, PCA_EUNSUPPORTED. */
+int pca_create(pca_ctx** out, int64_t M, int64_t N, int K, double eps, int max_iter, int algo);
+
+/* Tune / query the launch plan.  pca_set_option must be called before pca_workspace_bytes /
+ * pca_set_workspace; it re-plans and may return PCA_EUNSUPPORTED (e.g. forcing the resident path
+ * for a matrix that does not fit in shared memory). */
+int pca_set_option(pca_ctx*, int option, int64_t value);
+int pca_get_info(const pca_ctx*, int field, int64_t* value);
+
+/* Device workspace the caller must provide: the residual R (4*M*N bytes, first) followed by
+ * the partial-sum / exchange scratch of the persistent kernel. */
+size_t pca_workspace_bytes(const pca_ctx*);
+
+/* Hand the context a device buffer of at least pca_workspace_bytes() bytes, 256-byte aligned.
+ * The caller keeps ownership and must keep it alive while the context is used.
+ * Errors: PCA_EINVAL (NULL), PCA_EALIGN, PCA_EWORKSPACE (too small). */
+int pca_set_workspace(pca_ctx*, void* dev, size_t bytes);
+
+/* Step S0, mean centring, in place (eq. 1 / "each column is mean centered"):
+ *   mu_n = (1/M) sum_m X[m,n];  X[m,n] -= mu_n          (default: column means, C1)
+ * With PCA_OPT_CENTER_MODE = 1 the literal eq. (1) is applied instead (the mean COLUMN
+ * (1/N) sum_n X^(n) is subtracted from every column; listing PAPER.md:1009-1013).
+ *   X  dev, M x N, column-major ld = M, overwritten.
+ * Errors: PCA_EINVAL, PCA_EALIGN, PCA_ECUDA. */
+int pca_center(pca_ctx*, float* X, void* stream);
+
+/* The hot path: K components of NIPALS-PCA / GS-PCA on a centred X.
+ *   X       dev, M x N, ld = M, centred; never written (R <- X)
+ *   T       dev, M x K, ld = M, scores.  ||T[:,k]|| = lambda[k] for both algorithms
+ *           (NIPALS: t = R p; GS-PCA: T = V Lambda)
+ *   P       dev, N x K, ld = N, loadings with unit columns
+ *   lambda  dev, K floats, the last lambda' = ||T^(k)|| of each component (the paper's
+ *           "eigenvalue" = singular value of the centred X); extraction order
+ *   iters   dev, K int32, inner passes executed per component (1-based).  iters[k] == max_iter
+ *           means the test never fired (reported, not an error).  A component whose start
+ *           column, loads or scores have exactly zero norm returns lambda = 0, T = 0, P = 0,
+ *           iters = 0 (C7).
+ * After the stream is synchronised the residual R of eq. (4) is available via pca_residual.
+ * Sign: (T[:,k], P[:,k]) is defined up to a joint sign.
+ * Errors: PCA_EINVAL (NULL), PCA_EALIGN, PCA_EWORKSPACE, PCA_ECUDA. */
+int pca_run(pca_ctx*, const float* X, float* T, float* P, float* lambda, int32_t* iters, void* stream);
+
+/* Pointer to the residual R (dev, M x N, ld = M) inside the workspace; valid after a pca_run on
+ * this context has completed ("return T, P, R"). */
+int pca_residual(const pca_ctx*, const float** R);
+
+/* Convenience entry with HOST buffers (used for end-to-end timing): copies X (host, M x N,
+ * NOT centred) to the device, runs pca_center and pca_run on `stream`, copies T, P, lambda, iters
+ * back and synchronises the stream.  The context allocates private device staging buffers and
+ * the workspace on first use (freed by pca_destroy).  Host buffers should be pinned for full
+ * PCIe bandwidth but need not be.  Errors: as pca_center / pca_run. */
+int pca_fit_host(pca_ctx*, const float* X_host, float* T_host, float* P_host, float* lambda_host,
+                 int32_t* iters_host, void* stream);
+
+void pca_destroy(pca_ctx*);
+
+const char* pca_strerror(int code);
+
+/* cudaError_t (as int) of the last failing CUDA call on this context, 0 if none. */
+int pca_last_cuda_error(const pca_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PCA_H_ */

@@ -1,0 +1,387 @@
+// =====================================================================================
+// pca_api.cu -- host side of the C ABI declared in include/pca.h: argument checks, the launch
+// plan (path, CTAs, lane mapping, shared-memory carve-up, workspace layout) and the launches.
+// No torch types, no exceptions across the boundary, no printing.
+// =====================================================================================
+#include "../../include/pca.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "pca_center.cuh"
+#include "pca_solve.cuh"
+
+using pca::SolveParams;
+
+namespace {
+
+inline long long round_up(long long v, long long a) { return (v + a - 1) / a * a; }
+inline long long ceil_div(long long a, long long b) { return (a + b - 1) / b; }
+
+typedef void (*solve_kernel_t)(const SolveParams);
+
+struct Variant { int resident, vec, tr, rc; solve_kernel_t fn; };
+
+#define PCA_VARIANT(RES, VEC, TR, RC) {RES, VEC, TR, RC, pca::pca_solve_kernel<(RES != 0), VEC, TR, RC>}
+const Variant kVariants[] = {
+    PCA_VARIANT(0, 4, 32, 1), PCA_VARIANT(0, 4, 32, 2), PCA_VARIANT(0, 4, 32, 4),
+    PCA_VARIANT(0, 4, 8, 1),  PCA_VARIANT(0, 4, 8, 2),  PCA_VARIANT(0, 4, 8, 4),
+    PCA_VARIANT(0, 1, 32, 4),
+    PCA_VARIANT(1, 4, 32, 1), PCA_VARIANT(1, 4, 32, 2), PCA_VARIANT(1, 4, 32, 4),
+    PCA_VARIANT(1, 4, 8, 1),  PCA_VARIANT(1, 4, 8, 2),  PCA_VARIANT(1, 4, 8, 4),
+    PCA_VARIANT(1, 1, 32, 4),
+};
+#undef PCA_VARIANT
+
+}  // namespace
+
+struct pca_ctx {
+  long long M = 0, N = 0;
+  int K = 0;
+  double eps = 0;
+  int max_iter = 0;
+  int algo = 0;
+  // device
+  int device = 0, num_sms = 0, smem_optin = 0;
+  // options
+  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0;
+  // plan
+  bool planned = false;
+  int path = 0;  // 1 streaming, 2 resident
+  const Variant* variant = nullptr;
+  SolveParams prm{};
+  size_t smem_bytes = 0;
+  size_t ws_bytes = 0;
+  size_t ws_off_ppart = 0, ws_off_apart = 0, ws_off_bpart = 0, ws_off_pvec = 0, ws_off_qpart = 0, ws_off_spart = 0,
+         ws_off_bar = 0;
+  // workspace (caller-owned)
+  void* ws = nullptr;
+  size_t ws_given = 0;
+  bool ran = false;
+  // private staging for pca_fit_host
+  float *hX = nullptr, *hT = nullptr, *hP = nullptr, *hLam = nullptr;
+  int* hIters = nullptr;
+  void* hWs = nullptr;
+  int last_cuda = 0;
+};
+
+namespace {
+
+int cuda_fail(pca_ctx* c, cudaError_t e) {
+  c->last_cuda = (int)e;
+  return PCA_ECUDA;
+}
+#define PCA_CUDA(c, expr)                                \
+  do {                                                   \
+    cudaError_t e__ = (expr);                            \
+    if (e__ != cudaSuccess) return cuda_fail((c), e__);  \
+  } while (0)
+
+const Variant* find_variant(int resident, int vec, int tr, int rc) {
+  for (const Variant& v : kVariants)
+    if (v.resident == resident && v.vec == vec && v.tr == tr && v.rc == rc) return &v;
+  return nullptr;
+}
+
+// Lane mapping for a slab of `rv` row-vectors per column: smallest TR*RC >= rv (ties: wider TR),
+// else the largest mapping with a row-chunk loop.
+void choose_mapping(int vec, long long rv, int* tr, int* rc) {
+  if (vec == 1) { *tr = 32; *rc = 4; return; }
+  const int cand[6][2] = {{32, 1}, {32, 2}, {32, 4}, {8, 1}, {8, 2}, {8, 4}};
+  int best = -1;
+  long long best_cap = 0;
+  for (int i = 0; i < 6; ++i) {
+    const long long cap = (long long)cand[i][0] * cand[i][1];
+    if (cap >= rv && (best < 0 || cap < best_cap)) { best = i; best_cap = cap; }
+  }
+  if (best < 0) { *tr = 32; *rc = 4; return; }
+  *tr = cand[best][0];
+  *rc = cand[best][1];
+}
+
+// Fill prm's geometry + shared-memory carve-up for a given (path, G).  Returns dynamic smem bytes.
+size_t carve(pca_ctx* c, int resident, int G, int vec, SolveParams* p, int* tr, int* rc) {
+  const long long M = c->M, N = c->N;
+  p->G = G;
+  p->Mb = (int)round_up(ceil_div(M, G), vec);
+  p->Ns = (int)round_up(ceil_div(N, G), 4);
+  p->Gs = (int)ceil_div(N, p->Ns);
+  p->Npad = (int)round_up(N, 4);
+  p->Kpad = (int)round_up(c->K, 4);
+  p->slab_ld = resident ? (int)round_up(p->Mb, 4) : 0;
+  choose_mapping(vec, ceil_div(p->Mb, vec), tr, rc);
+  const int ch = vec * (*tr) * (*rc);
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 16); return (int)o; };
+  p->off_t = take((size_t)round_up(p->Mb, 4) * 4);
+  p->off_d = take((size_t)round_up(p->Mb, 4) * 4);
+  p->off_p = take((size_t)p->Npad * 4);
+  p->off_slice = take((size_t)p->Ns * 4);
+  p->off_coef = take((size_t)p->Kpad * 8);
+  p->off_lam = take((size_t)p->Kpad * 4);
+  p->off_scr = take((size_t)pca::kThreads * 8);
+  p->off_red = take((size_t)pca::kWarps * ch * 4);
+  p->off_slab = take(resident ? (size_t)p->slab_ld * (size_t)N * 4 : 0);
+  return off;
+}
+
+int make_plan(pca_ctx* c) {
+  c->planned = false;
+  const long long M = c->M, N = c->N;
+  const int vec = (M % 4 == 0) ? 4 : 1;
+  const int sms = c->num_sms;
+  // every slice owner handles at most kThreads columns
+  const int g_min = (int)ceil_div(N, pca::kThreads);
+  if (g_min > sms) return PCA_EUNSUPPORTED;
+
+  auto try_plan = [&](int resident, int G, SolveParams* p, const Variant** var, size_t* smem) -> bool {
+    if (G < g_min) G = g_min;
+    if (G > sms) G = sms;
+    if (G < 1) G = 1;
+    int tr, rc;
+    *smem = carve(c, resident, G, vec, p, &tr, &rc);
+    if (*smem > (size_t)c->smem_optin) return false;
+    *var = find_variant(resident, vec, tr, rc);
+    return *var != nullptr;
+  };
+
+  SolveParams p{};
+  const Variant* var = nullptr;
+  size_t smem = 0;
+  bool ok = false;
+  int path = 0;
+  const int want_path = c->opt_path;
+  if (want_path == 0 || want_path == 2) {
+    // resident: a single CTA if the whole matrix fits comfortably, else one CTA per SM
+    int G = c->opt_ctas > 0 ? c->opt_ctas : ((size_t)M * (size_t)N * 4 <= (size_t)160 * 1024 ? 1 : sms);
+    ok = try_plan(1, G, &p, &var, &smem);
+    if (!ok && c->opt_ctas == 0 && G != sms) ok = try_plan(1, sms, &p, &var, &smem);
+    if (ok) path = 2;
+    else if (want_path == 2) return PCA_EUNSUPPORTED;
+  }
+  if (!ok) {
+    int G = c->opt_ctas > 0 ? c->opt_ctas : sms;
+    ok = try_plan(0, G, &p, &var, &smem);
+    if (!ok) return PCA_EUNSUPPORTED;
+    path = 1;
+  }
+  // co-residency of the cooperative grid
+  cudaError_t e = cudaFuncSetAttribute(var->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, var->fn, pca::kThreads, smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
+
+  p.M = M; p.N = N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  // workspace layout: R first
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
+  take((size_t)M * (size_t)N * 4);
+  c->ws_off_ppart = take((size_t)p.G * p.Npad * 4);
+  c->ws_off_apart = take((size_t)p.Gs * p.Kpad * 8);
+  c->ws_off_bpart = take((size_t)p.G * p.Kpad * 8);
+  c->ws_off_pvec = take((size_t)p.Npad * 4);
+  c->ws_off_qpart = take((size_t)p.Gs * 8);
+  c->ws_off_spart = take((size_t)p.G * 8);
+  c->ws_off_bar = take(256);
+  c->ws_bytes = off;
+  c->prm = p;
+  c->variant = var;
+  c->smem_bytes = smem;
+  c->path = path;
+  c->planned = true;
+  c->ws = nullptr;  // a new plan invalidates a previously set workspace
+  c->ws_given = 0;
+  c->ran = false;
+  return PCA_OK;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+int pca_create(pca_ctx** out, int64_t M, int64_t N, int K, double eps, int max_iter, int algo) {
+  if (!out) return PCA_EINVAL;
+  *out = nullptr;
+  if (M < 1 || N < 1 || K < 1 || (int64_t)K > N || !(eps >= 0.0) || max_iter < 1) return PCA_EINVAL;
+  if (algo != PCA_ALGO_NIPALS && algo != PCA_ALGO_GS) return PCA_EINVAL;
+  if (N > (int64_t)1 << 30 || M > (int64_t)1 << 40) return PCA_EUNSUPPORTED;
+  pca_ctx* c = new (std::nothrow) pca_ctx();
+  if (!c) return PCA_EINVAL;
+  c->M = M; c->N = N; c->K = K; c->eps = eps; c->max_iter = max_iter; c->algo = algo;
+  cudaError_t e = cudaGetDevice(&c->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
+  int coop = 0;
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
+  if (e != cudaSuccess || !coop) {
+    delete c;
+    return PCA_ECUDA;  // no CUDA device: there is no CPU fallback
+  }
+  const int rc = make_plan(c);
+  if (rc != PCA_OK) {
+    delete c;
+    return rc;
+  }
+  *out = c;
+  return PCA_OK;
+}
+
+int pca_set_option(pca_ctx* c, int option, int64_t value) {
+  if (!c) return PCA_EINVAL;
+  switch (option) {
+    case PCA_OPT_PATH:
+      if (value < 0 || value > 2) return PCA_EINVAL;
+      c->opt_path = (int)value;
+      break;
+    case PCA_OPT_CTAS:
+      if (value < 0 || value > c->num_sms) return PCA_EINVAL;
+      c->opt_ctas = (int)value;
+      break;
+    case PCA_OPT_CENTER_MODE:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_center_mode = (int)value;
+      return PCA_OK;
+    default:
+      return PCA_EINVAL;
+  }
+  return make_plan(c);
+}
+
+int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
+  if (!c || !value || !c->planned) return PCA_EINVAL;
+  switch (field) {
+    case PCA_INFO_PATH: *value = c->path; break;
+    case PCA_INFO_CTAS: *value = c->prm.G; break;
+    case PCA_INFO_THREADS: *value = pca::kThreads; break;
+    case PCA_INFO_SMEM_BYTES: *value = (int64_t)c->smem_bytes; break;
+    case PCA_INFO_ROWS_PER_CTA: *value = c->prm.Mb; break;
+    case PCA_INFO_LAUNCHES_PER_RUN: *value = 1; break;
+    case PCA_INFO_NUM_SMS: *value = c->num_sms; break;
+    default: return PCA_EINVAL;
+  }
+  return PCA_OK;
+}
+
+size_t pca_workspace_bytes(const pca_ctx* c) { return (c && c->planned) ? c->ws_bytes : 0; }
+
+int pca_set_workspace(pca_ctx* c, void* dev, size_t bytes) {
+  if (!c || !dev || !c->planned) return PCA_EINVAL;
+  if ((reinterpret_cast<uintptr_t>(dev) & 255u) != 0) return PCA_EALIGN;
+  if (bytes < c->ws_bytes) return PCA_EWORKSPACE;
+  c->ws = dev;
+  c->ws_given = bytes;
+  c->ran = false;
+  return PCA_OK;
+}
+
+int pca_center(pca_ctx* c, float* X, void* stream) {
+  if (!c || !X) return PCA_EINVAL;
+  if (!aligned16(X)) return PCA_EALIGN;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (c->opt_center_mode == 0) {
+    const int grid = (int)(c->N < (long long)c->num_sms * 4 ? c->N : (long long)c->num_sms * 4);
+    pca::pca_center_columns_kernel<<<grid, pca::kCenterThreads, 0, st>>>(X, c->M, (int)c->N, (c->M % 4 == 0) ? 1 : 0);
+  } else {
+    const long long grid = (c->M + 255) / 256;
+    pca::pca_center_eq1_kernel<<<(unsigned)grid, 256, 0, st>>>(X, c->M, (int)c->N);
+  }
+  PCA_CUDA(c, cudaGetLastError());
+  return PCA_OK;
+}
+
+int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32_t* iters, void* stream) {
+  if (!c || !X || !T || !P || !lambda || !iters || !c->planned) return PCA_EINVAL;
+  if (!aligned16(X) || !aligned16(T) || !aligned16(P)) return PCA_EALIGN;
+  if (!c->ws || c->ws_given < c->ws_bytes) return PCA_EWORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  unsigned char* ws = static_cast<unsigned char*>(c->ws);
+  SolveParams p = c->prm;
+  p.X = X;
+  p.R = reinterpret_cast<float*>(ws);
+  p.T = T; p.P = P; p.lambda = lambda; p.iters = iters;
+  p.Ppart = reinterpret_cast<float*>(ws + c->ws_off_ppart);
+  p.Apart = reinterpret_cast<double*>(ws + c->ws_off_apart);
+  p.Bpart = reinterpret_cast<double*>(ws + c->ws_off_bpart);
+  p.pvec = reinterpret_cast<float*>(ws + c->ws_off_pvec);
+  p.qpart = reinterpret_cast<double*>(ws + c->ws_off_qpart);
+  p.spart = reinterpret_cast<double*>(ws + c->ws_off_spart);
+  p.bar = reinterpret_cast<unsigned long long*>(ws + c->ws_off_bar);
+  PCA_CUDA(c, cudaMemsetAsync(p.bar, 0, 256, st));
+  void* args[] = {&p};
+  PCA_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(c->variant->fn), dim3((unsigned)p.G),
+                                          dim3(pca::kThreads), args, c->smem_bytes, st));
+  c->ran = true;
+  return PCA_OK;
+}
+
+int pca_residual(const pca_ctx* c, const float** R) {
+  if (!c || !R) return PCA_EINVAL;
+  if (!c->ws || !c->ran) return PCA_EWORKSPACE;
+  *R = reinterpret_cast<const float*>(c->ws);
+  return PCA_OK;
+}
+
+int pca_fit_host(pca_ctx* c, const float* X_host, float* T_host, float* P_host, float* lambda_host,
+                 int32_t* iters_host, void* stream) {
+  if (!c || !X_host || !T_host || !P_host || !lambda_host || !iters_host || !c->planned) return PCA_EINVAL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const size_t xb = (size_t)c->M * (size_t)c->N * 4, tb = (size_t)c->M * c->K * 4, pb = (size_t)c->N * c->K * 4;
+  if (!c->hX) {
+    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hX), xb));
+    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hT), tb));
+    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hP), pb));
+    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hLam), (size_t)c->K * 4));
+    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hIters), (size_t)c->K * 4));
+  }
+  if (!c->ws) {
+    if (!c->hWs) PCA_CUDA(c, cudaMalloc(&c->hWs, c->ws_bytes));
+    c->ws = c->hWs;
+    c->ws_given = c->ws_bytes;
+  }
+  PCA_CUDA(c, cudaMemcpyAsync(c->hX, X_host, xb, cudaMemcpyHostToDevice, st));
+  int rc = pca_center(c, c->hX, stream);
+  if (rc != PCA_OK) return rc;
+  rc = pca_run(c, c->hX, c->hT, c->hP, c->hLam, c->hIters, stream);
+  if (rc != PCA_OK) return rc;
+  PCA_CUDA(c, cudaMemcpyAsync(T_host, c->hT, tb, cudaMemcpyDeviceToHost, st));
+  PCA_CUDA(c, cudaMemcpyAsync(P_host, c->hP, pb, cudaMemcpyDeviceToHost, st));
+  PCA_CUDA(c, cudaMemcpyAsync(lambda_host, c->hLam, (size_t)c->K * 4, cudaMemcpyDeviceToHost, st));
+  PCA_CUDA(c, cudaMemcpyAsync(iters_host, c->hIters, (size_t)c->K * 4, cudaMemcpyDeviceToHost, st));
+  PCA_CUDA(c, cudaStreamSynchronize(st));
+  return PCA_OK;
+}
+
+void pca_destroy(pca_ctx* c) {
+  if (!c) return;
+  if (c->hX) cudaFree(c->hX);
+  if (c->hT) cudaFree(c->hT);
+  if (c->hP) cudaFree(c->hP);
+  if (c->hLam) cudaFree(c->hLam);
+  if (c->hIters) cudaFree(c->hIters);
+  if (c->hWs) cudaFree(c->hWs);
+  delete c;
+}
+
+const char* pca_strerror(int code) {
+  switch (code) {
+    case PCA_OK: return "ok";
+    case PCA_EINVAL: return "invalid argument";
+    case PCA_EALIGN: return "device pointer not sufficiently aligned";
+    case PCA_ECUDA: return "CUDA runtime error (no device, or a launch/copy failed)";
+    case PCA_EWORKSPACE: return "workspace missing or too small";
+    case PCA_EUNSUPPORTED: return "shape not supported by this build";
+    default: return "unknown error";
+  }
+}
+
+int pca_last_cuda_error(const pca_ctx* c) { return c ? c->last_cuda : 0; }
+
+}  // extern "C"

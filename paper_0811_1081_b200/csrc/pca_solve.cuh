@@ -1,0 +1,266 @@
+// =====================================================================================
+// pca_solve.cuh -- the persistent, grid-synchronised solve kernel: all K components, all inner
+// passes, convergence tested on the device (no host round-trip), one launch per pca_run.
+//
+// Per component k (statement order of PAPER.md:555-568 / :1016-1038):
+//   S1  t <- column k of the deflated residual
+//   loop (at most max_iter passes):
+//     Ph1  S2  partial loads  pp_b = R_b^T t_b                (first pass of a component also
+//              applies the previous component's deflation S9, or the copy R <- X for k = 0)
+//     ---- grid barrier ----
+//     Ph2      column-slice owners sum the G partials -> p~ ;  GS-PCA: A-partials  P_(k)^T p~   (S3)
+//     ---- grid barrier (GS-PCA, k > 0) ----
+//     Ph3      GS-PCA: A = sum of partials;  p^ = p~ - P_(k) A ;  ||p^||^2 partials            (S3, S4)
+//     ---- grid barrier ----
+//     Ph4  S4  p = p^ / ||p^|| ;  S5  t_b = R_b p ;  GS-PCA: B-partials V_(k)^T t               (S6)
+//     ---- grid barrier (GS-PCA, k > 0) ----
+//     Ph5      GS-PCA: B = sum of partials;  t_b -= V_b B ;  ||t||^2 partials                   (S6, S7)
+//     ---- grid barrier ----
+//     Ph6  S7  lambda' = ||t|| ;  GS-PCA: t /= lambda' ;  S8 test |lambda - lambda'| < eps lambda'
+//   store T[:,k], P[:,k], lambda[k], iters[k];  d <- (GS ? lambda' v : t) for the next deflation
+// after the last component: final deflation (R of eq. 4) and GS-PCA's T <- V Lambda (S10).
+// =====================================================================================
+#pragma once
+#include "pca_device.cuh"
+
+namespace pca {
+
+struct SolveParams {
+  const float* X;        // M x N centred input (never written)
+  float* R;              // M x N residual workspace
+  float* T;              // M x K
+  float* P;              // N x K
+  float* lambda;         // K
+  int* iters;            // K
+  long long M, N;
+  int K;
+  double eps;
+  int max_iter;
+  int algo;              // 0 NIPALS, 1 GS
+  int G;                 // CTAs
+  int Mb;                // rows per CTA (uniform; last CTAs may own fewer / none)
+  int Ns;                // columns per slice owner (multiple of 4)
+  int Gs;                // number of slice owners = ceil(N / Ns) <= G
+  int slab_ld;           // resident path: column stride of the SMEM slab (floats)
+  int Npad;              // row stride of Ppart (floats)
+  int Kpad;              // row stride of Apart / Bpart (doubles)
+  float* Ppart;          // [G][Npad]   partial loads
+  double* Apart;         // [Gs][Kpad]  partial A (loads-side GS coefficients)
+  double* Bpart;         // [G][Kpad]   partial B (scores-side GS coefficients)
+  float* pvec;           // [Npad]      p^ (orthogonalised, not yet normalised)
+  double* qpart;         // [Gs]        ||p^||^2 partials
+  double* spart;         // [G]         ||t||^2 partials
+  unsigned long long* bar;  // grid barrier counter (zeroed before launch)
+  // shared memory carve-up (bytes from the start of dynamic smem), computed by the host plan
+  int off_t, off_d, off_p, off_slice, off_coef, off_lam, off_scr, off_red, off_slab;
+};
+
+template <bool RESIDENT, int VEC, int TR, int RC>
+__global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParams prm) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  float* t_s = reinterpret_cast<float*>(smem + prm.off_t);          // Mb: this CTA's rows of t / v
+  float* d_s = reinterpret_cast<float*>(smem + prm.off_d);          // Mb: deflation vector rows
+  float* p_s = reinterpret_cast<float*>(smem + prm.off_p);          // N : full loads vector
+  float* slice_s = reinterpret_cast<float*>(smem + prm.off_slice);  // Ns: this CTA's slice of p~ / p^
+  double* coef_s = reinterpret_cast<double*>(smem + prm.off_coef);  // K : A or B
+  float* lam_s = reinterpret_cast<float*>(smem + prm.off_lam);      // K : lambda_k (GS final scaling)
+  double* scr = reinterpret_cast<double*>(smem + prm.off_scr);      // kThreads doubles scratch
+  float* red_s = reinterpret_cast<float*>(smem + prm.off_red);      // kWarps * CH floats
+  float* slab = reinterpret_cast<float*>(smem + prm.off_slab);      // resident slab [N][slab_ld]
+
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int b = blockIdx.x;
+  const long long M = prm.M;
+  const int N = (int)prm.N, K = prm.K, G = prm.G;
+  const bool gs = prm.algo == 1;
+  const long long m0 = (long long)b * prm.Mb;
+  const int mb = (int)max(0LL, min((long long)prm.Mb, M - m0));
+  const int n0 = b * prm.Ns;
+  const int ns = max(0, min(prm.Ns, N - n0));
+  const int slab_ld = prm.slab_ld;
+  unsigned long long bar_target = 0;
+
+  const float* Xb = prm.X + m0;          // row-offset views (column stride M)
+  float* Rb = prm.R + m0;
+  float* Tb = prm.T + m0;
+  float* my_part = prm.Ppart + (size_t)b * prm.Npad;
+
+  for (int i = tid; i < prm.Mb; i += kThreads) d_s[i] = 0.f;
+  for (int n = tid; n < N; n += kThreads) p_s[n] = 0.f;
+  __syncthreads();
+
+  for (int k = 0; k < K; ++k) {
+    // ---- S1: t <- R^(k) of the deflated residual (reading C6) ----
+    for (int i = tid; i < mb; i += kThreads) {
+      float r;
+      if (k == 0) r = ld_cg(Xb + i);                                   // R <- X not yet materialised
+      else if constexpr (RESIDENT) r = slab[(size_t)k * slab_ld + i];
+      else r = ld_cg(Rb + (size_t)k * M + i);
+      t_s[i] = fmaf(-d_s[i], p_s[k], r);                               // pending deflation of comp k-1
+    }
+    __syncthreads();
+
+    double lam = 0.0, lam_new = 0.0;
+    int it = 0;
+    bool degenerate = false;
+    for (int j = 0; j < prm.max_iter; ++j) {
+      // ---- Ph1: partial loads (S2), fused with deflation / copy on the first pass (S9, A2) ----
+      if (j == 0) {
+        if constexpr (RESIDENT) {
+          if (k == 0) pass_t<VEC, TR, RC, SRC_GLOBAL, DST_SLAB, true, true>(Xb, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+          else        pass_t<VEC, TR, RC, SRC_SLAB, DST_SLAB, true, true>(nullptr, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+        } else {
+          pass_t<VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, true>(k == 0 ? Xb : Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
+        }
+      } else {
+        if constexpr (RESIDENT) pass_t<VEC, TR, RC, SRC_SLAB, DST_NONE, false, true>(nullptr, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+        else                    pass_t<VEC, TR, RC, SRC_GLOBAL, DST_NONE, false, true>(Rb, nullptr, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
+      }
+      if (mb == 0) for (int n = tid; n < N; n += kThreads) my_part[n] = 0.f;   // CTA without rows
+      grid_barrier(prm.bar, bar_target, G);
+
+      // ---- Ph2: slice owners reduce the G partials: p~[n] = sum_b pp_b[n] ----
+      if (ns > 0) {
+        const int nsub = min(kThreads / ns, G);
+        const int sub = tid / ns, i = tid - sub * ns;
+        double v = 0.0;
+        if (sub < nsub)
+          for (int bb = sub; bb < G; bb += nsub) v += (double)ld_cg(prm.Ppart + (size_t)bb * prm.Npad + n0 + i);
+        if (sub < nsub) scr[sub * ns + i] = v;
+        __syncthreads();
+        if (tid < ns) {
+          double s = 0.0;
+          for (int q = 0; q < nsub; ++q) s += scr[q * ns + tid];
+          slice_s[tid] = (float)s;
+        }
+        __syncthreads();
+      }
+      if (gs && k > 0) {
+        // ---- S3: A-partials  a_b[jj] = sum_{n in slice} P[n,jj] p~[n] ----
+        if (ns > 0) {
+          for (int jj = tid; jj < k; jj += kThreads) {
+            const float* pj = prm.P + (size_t)jj * N + n0;
+            double a = 0.0;
+            for (int i = 0; i < ns; ++i) a += (double)ld_cg(pj + i) * (double)slice_s[i];
+            prm.Apart[(size_t)b * prm.Kpad + jj] = a;
+          }
+        }
+        grid_barrier(prm.bar, bar_target, G);
+        // ---- Ph3: A = sum of partials;  p^ = p~ - P_(k) A ----
+        if (ns > 0) {
+          reduce_coef_parts(coef_s, prm.Apart, k, prm.Gs, prm.Kpad, scr);
+          const int nsub = kThreads / ns;
+          const int sub = tid / ns, i = tid - sub * ns;
+          double v = 0.0;
+          if (sub < nsub)
+            for (int jj = sub; jj < k; jj += nsub) v += (double)ld_cg(prm.P + (size_t)jj * N + n0 + i) * coef_s[jj];
+          __syncthreads();
+          if (sub < nsub) scr[sub * ns + i] = v;
+          __syncthreads();
+          if (tid < ns) {
+            double s = 0.0;
+            for (int q = 0; q < nsub; ++q) s += scr[q * ns + tid];
+            slice_s[tid] = (float)((double)slice_s[tid] - s);
+          }
+          __syncthreads();
+        }
+      }
+      // ---- S4 (first half): ||p^||^2 partial, publish the slice ----
+      if (ns > 0) {
+        double q = 0.0;
+        if (tid < ns) {
+          const float v = slice_s[tid];
+          prm.pvec[n0 + tid] = v;
+          q = (double)v * (double)v;
+        }
+        q = block_sum(q, scr);
+        if (tid == 0) prm.qpart[b] = q;
+      }
+      grid_barrier(prm.bar, bar_target, G);
+
+      // ---- Ph4: p = p^/||p^||;  S5: t = R p ----
+      const double pn2 = sum_parts(prm.qpart, prm.Gs, scr);
+      if (!(pn2 > 0.0)) { degenerate = true; break; }                 // reading C7 (uniform across CTAs)
+      const float inv_pn = (float)(1.0 / sqrt(pn2));
+      for (int n = tid; n < N; n += kThreads) p_s[n] = ld_cg(prm.pvec + n) * inv_pn;
+      __syncthreads();
+      if constexpr (RESIDENT) pass_n<VEC, TR, RC, SRC_SLAB>(nullptr, M, slab, slab_ld, mb, N, p_s, t_s, red_s);
+      else                    pass_n<VEC, TR, RC, SRC_GLOBAL>(Rb, M, nullptr, 0, mb, N, p_s, t_s, red_s);
+
+      if (gs && k > 0) {
+        // ---- S6: B-partials  b_b[jj] = sum_{rows} V[m,jj] t[m] ----
+        for (int jj = w; jj < k; jj += kWarps) {
+          const float* vj = Tb + (size_t)jj * M;
+          float a = 0.f;
+          for (int i = lane; i < mb; i += 32) a = fmaf(ld_cg(vj + i), t_s[i], a);
+          const double s = warp_sum((double)a);
+          if (lane == 0) prm.Bpart[(size_t)b * prm.Kpad + jj] = s;
+        }
+        grid_barrier(prm.bar, bar_target, G);
+        // ---- Ph5: B = sum of partials;  t -= V_(k) B ----
+        reduce_coef_parts(coef_s, prm.Bpart, k, G, prm.Kpad, scr);
+        for (int i = tid; i < mb; i += kThreads) {
+          float corr = 0.f;
+          for (int jj = 0; jj < k; ++jj) corr = fmaf(ld_cg(Tb + (size_t)jj * M + i), (float)coef_s[jj], corr);
+          t_s[i] -= corr;
+        }
+        __syncthreads();
+      }
+      // ---- S7: lambda' = ||t|| ----
+      {
+        double s = 0.0;
+        for (int i = tid; i < mb; i += kThreads) { const double v = (double)t_s[i]; s += v * v; }
+        s = block_sum(s, scr);
+        if (tid == 0) prm.spart[b] = s;
+      }
+      grid_barrier(prm.bar, bar_target, G);
+      const double l2 = sum_parts(prm.spart, G, scr);
+      if (!(l2 > 0.0)) { degenerate = true; break; }                  // reading C7
+      lam_new = sqrt(l2);
+      if (gs) {                                                       // V^(k) <- V^(k)/lambda_k
+        const float inv = (float)(1.0 / lam_new);
+        for (int i = tid; i < mb; i += kThreads) t_s[i] *= inv;
+        __syncthreads();
+      }
+      it = j + 1;
+      // ---- S8: listings' strict relative test (reading C3) ----
+      if (fabs(lam - lam_new) < prm.eps * lam_new) break;
+      lam = lam_new;
+    }
+
+    // ---- component done: store, and set up the pending deflation ----
+    if (degenerate) {
+      for (int i = tid; i < mb; i += kThreads) { Tb[(size_t)k * M + i] = 0.f; d_s[i] = 0.f; t_s[i] = 0.f; }
+      if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = 0.f;
+      if (b == 0 && tid == 0) { prm.lambda[k] = 0.f; prm.iters[k] = 0; }
+      if (tid == 0) lam_s[k] = 0.f;
+    } else {
+      const float lamf = (float)lam_new;
+      for (int i = tid; i < mb; i += kThreads) {
+        const float v = t_s[i];
+        Tb[(size_t)k * M + i] = v;                                    // GS-PCA: unit v until the final scaling
+        d_s[i] = gs ? lamf * v : v;                                   // R -= lambda v p^T / R -= t p^T
+      }
+      if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = p_s[n0 + tid];
+      if (b == 0 && tid == 0) { prm.lambda[k] = lamf; prm.iters[k] = it; }
+      if (tid == 0) lam_s[k] = lamf;
+    }
+    __syncthreads();
+  }
+
+  // ---- final deflation: the residual R of eq. (4) ----
+  if constexpr (RESIDENT)
+    pass_t<VEC, TR, RC, SRC_SLAB, DST_GLOBAL, true, false>(nullptr, Rb, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+  else
+    pass_t<VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, false>(Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
+  // ---- S10: GS-PCA  T <- V Lambda ----
+  if (gs) {
+    __syncthreads();
+    for (int kk = 0; kk < K; ++kk) {
+      const float l = lam_s[kk];
+      for (int i = tid; i < mb; i += kThreads) Tb[(size_t)kk * M + i] *= l;
+    }
+  }
+}
+
+}  // namespace pca

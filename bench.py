@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the iterative-PCA hot path on B200 (driver contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+           --master-port P bench.py --gpus N --steps K --warmup W
+
+One "step" = one pass of the whole hot path over one seeded synthetic problem already resident
+in HBM: S0 `pca_center` on a fresh copy of the raw matrix, then `pca_run` (all K components: every
+inner pass S2-S8, the fused deflations S9, the epilogue S10).  The default workload is
+BASELINE.json configs[3] (M=65536 x N=2048, K=128, GS-PCA, eps=1e-7): the HBM-resident
+configuration the metric's HBM roofline -- and the north_star's ">= 70 % of HBM bandwidth"
+target -- is quoted on (DESIGN.md section 9 says why not configs[1]); configs[1] is measured in
+the same run and reported under "also".
+
+Rank 0 prints ONE JSON line.  `--impl reference` times the CPU oracle (oracle/, as it stands) on
+a bounded sample of the same workload instead (this tier's reference arm).
+
+This file may execute oracle/ only in the `cpu_baseline` leg and under `--impl reference`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_0811_1081_b200 import inputs  # noqa: E402  (seeded generators only; no method arithmetic)
+
+METRIC = "PCA components/s"
+UNIT = "components/s"
+WORKLOADS = {f"cfg{i + 1}": i for i in range(len(inputs.CONFIGS))}
+L2_BYTES = 126 * 1024 * 1024
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic bytes
+# ------------------------------------------------------------------------------------------------
+def bytes_per_inner_iteration(M, N, k, gs):
+    """Two reads of R, one read of each Gram-Schmidt panel, t and p written once and read once."""
+    return 8 * M * N + (4 * k * (M + N) if gs else 0) + 8 * (M + N)
+
+
+def algorithmic_bytes(M, N, iters, gs):
+    """What one pca_run must move for the pass counts `iters` it actually executed: the inner
+    iterations, + per component the extra WRITE of R of the fused deflation (4MN), + the final
+    deflation pass that materialises the residual of eq. (4) (read + write, 8MN)."""
+    total = 0
+    for k, it in enumerate(iters):
+        total += int(it) * bytes_per_inner_iteration(M, N, k, gs) + 4 * M * N
+    return total + 8 * M * N
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU through NVML every 100 ms."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+               0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index):
+        self.sm, self.reasons, self.max_mhz, self.power = [], set(), None, 0.0
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # noqa: BLE001
+            self._nv = None
+            self.error = repr(e)
+
+    def _loop(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                self.power = max(self.power, nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "NVML unavailable"}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.sm), "power_w_max": round(self.power, 1)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+class GpuProblem:
+    """Device buffers + context of one workload (torch: memory and streams only)."""
+
+    def __init__(self, cfg, algo, X_np, K=None, eps=None, max_iter=None):
+        import torch
+        from paper_0811_1081_b200 import binding
+        self.torch, self.binding, self.cfg, self.algo = torch, binding, cfg, algo
+        self.M, self.N = cfg.M, cfg.N
+        self.K = K or cfg.K
+        self.eps = cfg.eps if eps is None else eps
+        self.max_iter = max_iter or cfg.max_iter
+        self.ctx = binding.PcaContext(self.M, self.N, self.K, self.eps, self.max_iter, algo)
+        self.X_raw = binding.from_colmajor(X_np)
+        self.X = torch.empty_like(self.X_raw)
+        self.T = torch.empty((self.K, self.M), dtype=torch.float32, device="cuda")
+        self.P = torch.empty((self.K, self.N), dtype=torch.float32, device="cuda")
+        self.lam = torch.empty(self.K, dtype=torch.float32, device="cuda")
+        self.iters = torch.empty(self.K, dtype=torch.int32, device="cuda")
+        self.ctx.ensure_workspace()
+        self.flush = None
+        if 4 * self.M * self.N <= 2 * L2_BYTES:                 # inputs not larger than L2: flush between steps
+            self.flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device="cuda")
+
+    def step(self):
+        """Enqueue one step; returns (event pair of the step, event pair of the solve kernel)."""
+        e = [self.torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        if self.flush is not None:
+            self.flush.fill_(1)
+        e[0].record()
+        self.X.copy_(self.X_raw)
+        self.ctx.pca_center(self.X)
+        e[2].record()
+        self.ctx.pca_run(self.X, self.T, self.P, self.lam, self.iters)
+        e[3].record()
+        e[1].record()
+        return e
+
+    def launches_per_step(self):
+        return 1 + self.ctx.pca_get_info(self.binding.PCA_INFO_LAUNCHES_PER_RUN)   # pca_center + pca_run
+
+    def gs(self):
+        return self.algo == inputs.ALGO_GS
+
+
+def time_steps(prob, steps, warmup):
+    torch = prob.torch
+    for _ in range(warmup):
+        prob.step()
+    torch.cuda.synchronize()
+    evs = [prob.step() for _ in range(steps)]
+    torch.cuda.synchronize()
+    step_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    run_ms = [e[2].elapsed_time(e[3]) for e in evs]
+    return step_ms, run_ms
+
+
+def roofline(prob, run_ms_mean, peaks):
+    iters = prob.iters.cpu().numpy()
+    nbytes = algorithmic_bytes(prob.M, prob.N, iters, prob.gs())
+    achieved = nbytes / (run_ms_mean * 1e-3) / 1e9
+    peak = peaks["hbm_gbs"]
+    total_iters = int(iters.sum())
+    return {
+        "bound": "hbm", "kernel": "pca_solve_kernel (persistent; all passes of all components in one launch)",
+        "achieved": round(achieved, 1), "peak": peak, "peak_source": peaks["source"], "unit": "GB/s",
+        "frac": round(achieved / peak, 4), "traffic": peaks.get("traffic"),
+        "algorithmic_bytes_per_launch": int(nbytes), "inner_iterations_per_launch": total_iters,
+        "us_per_inner_iteration": round(run_ms_mean * 1e3 / max(total_iters, 1), 3),
+        "bytes_model": "8MN + [GS]4k(M+N) + 8(M+N) per inner iteration, + 4MN per component, + 8MN final deflation",
+    }, iters
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "MEASURED_PEAKS.json hbm_gbs (measured copy bandwidth)"}
+    return {"hbm_gbs": 6650.0, "source": "fallback 6.65 TB/s (B200_PROFILING.md; MEASURED_PEAKS.json absent)"}
+
+
+def e2e_leg(prob, X_np, steps):
+    """Same metric through the C-ABI call with HOST buffers: H2D of X, centring, solve, D2H of T, P, lambda, iters."""
+    torch = prob.torch
+    Xh = torch.from_numpy(np.ascontiguousarray(X_np.T)).pin_memory()
+    Th = torch.empty((prob.K, prob.M), dtype=torch.float32).pin_memory()
+    Ph = torch.empty((prob.K, prob.N), dtype=torch.float32).pin_memory()
+    lh = torch.empty(prob.K, dtype=torch.float32).pin_memory()
+    ih = torch.empty(prob.K, dtype=torch.int32).pin_memory()
+    prob.ctx.pca_fit_host(Xh, Th, Ph, lh, ih)                   # warm-up (allocates the staging buffers)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        prob.ctx.pca_fit_host(Xh, Th, Ph, lh, ih)               # synchronises the stream itself
+    dt = (time.perf_counter() - t0) / steps
+    return dt, 4 * prob.M * prob.N, 4 * prob.K * (prob.M + prob.N) + 8 * prob.K
+
+
+def cpu_baseline_leg(cfg, algo, X_np, budget_s=20.0):
+    """The oracle as it stands, on this box's host cores, on a bounded sample of the workload:
+    the first components of the full-size problem (components are extracted one after the other,
+    so the first k_s components of the K-component solve ARE the k_s-component solve)."""
+    import oracle
+    Xc = oracle.center(X_np)
+    t0 = time.perf_counter()
+    r = oracle.pca(Xc, 1, cfg.eps, cfg.max_iter, algo, want_residual=False)
+    t1 = time.perf_counter() - t0
+    ks, t, its = 1, t1, int(r.iters.sum())
+    more = int(min(cfg.K, budget_s / max(t1, 1e-3)))
+    if more >= 2:                                               # cheap problem: a longer prefix
+        t0 = time.perf_counter()
+        r = oracle.pca(Xc, more, cfg.eps, cfg.max_iter, algo, want_residual=False)
+        t, ks, its = time.perf_counter() - t0, more, int(r.iters.sum())
+    return {"value": round(ks / t, 4), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"first {ks} of {cfg.K} components of {cfg.name} at full size ({its} inner iterations, "
+                      f"{t:.1f} s, float64, eps={cfg.eps:g})",
+            "us_per_inner_iteration": round(t / max(its, 1) * 1e6, 1)}
+
+
+def pick_algo(cfg):
+    return inputs.ALGO_GS if inputs.ALGO_GS in cfg.algos else cfg.algos[0]
+
+
+def run_cuda_arm(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_0811_1081_b200 import binding
+    binding.load_library()
+
+    ci = WORKLOADS[args.workload]
+    cfg = inputs.config(ci)
+    algo = pick_algo(cfg)
+    K = args.components or cfg.K
+    eps, max_iter = (0.0, args.fixed_iters) if args.fixed_iters else (cfg.eps, cfg.max_iter)
+    pr = inputs.generate(cfg)                                   # replicas only: every rank solves the same seeded problem
+    prob = GpuProblem(cfg, algo, pr.X, K=K, eps=eps, max_iter=max_iter)
+    peaks = load_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        prob.step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    t_wall = time.perf_counter()
+    evs = [prob.step() for _ in range(args.steps)]
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop()
+    step_ms = float(np.sum([e[0].elapsed_time(e[1]) for e in evs]))
+    run_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
+    if world > 1:
+        tt = torch.tensor([step_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        step_ms = float(tt.item())
+    ms_per_step = step_ms / args.steps
+    value = world * K / (ms_per_step * 1e-3)
+    roof, iters = roofline(prob, run_ms, peaks)
+
+    out = None
+    if rank == 0:
+        info = prob.ctx.info()
+        out = {
+            "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {
+                "workload": f"BASELINE.json configs[{ci}] {cfg.name}: M={cfg.M} N={cfg.N} K={K} "
+                            f"{'GS-PCA' if algo == inputs.ALGO_GS else 'NIPALS-PCA'} eps={eps:g} max_iter={max_iter}",
+                "recipe": f"{cfg.kind} {cfg.spectrum} noise_std={cfg.noise:g} seed={cfg.seed} ({cfg.note})",
+                "parallelism": "replicas only (one independent problem per GPU)" if world > 1 else "single GPU",
+                "l2": "input (4MN bytes) larger than L2" if prob.flush is None else "L2 flushed (252 MiB write) between steps",
+                "plan": info,
+            },
+            "gpu_launches": args.steps * prob.launches_per_step(),
+            "wall_s_timed_region": round(t_wall, 3),
+            "clocks": clocks,
+            "roofline": roof,
+            "inner_iterations": {"total": int(iters.sum()), "max_per_component": int(iters.max()),
+                                 "hit_max_iter": int((iters >= max_iter).sum()) if not args.fixed_iters else None},
+        }
+    # ---- e2e: host buffers through pca_fit_host (every rank, max over ranks) ----
+    if not args.no_e2e:
+        dt, h2d, d2h = e2e_leg(prob, pr.X, max(1, min(args.steps, args.e2e_steps)))
+        if world > 1:
+            tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        if rank == 0:
+            out["e2e"] = {"value": round(world * K / dt, 3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                          "d2h_bytes_per_step": d2h, "ms_per_step": round(dt * 1e3, 3),
+                          "api": "pca_fit_host (pinned host X in; T, P, lambda, iters out)"}
+    # ---- configs[1] measured beside it (cheap: ~10 ms per solve) ----
+    if rank == 0 and not args.no_also and not args.fixed_iters and args.workload != "cfg2":
+        del prob
+        torch.cuda.empty_cache()
+        c2 = inputs.config(1)
+        p2 = inputs.generate(c2)
+        q = GpuProblem(c2, inputs.ALGO_GS, p2.X)
+        s_ms, r_ms = time_steps(q, 5, 3)
+        roof2, it2 = roofline(q, float(np.mean(r_ms)), peaks)
+        out["also"] = [{"workload": f"BASELINE.json configs[1] {c2.name} K={c2.K} GS-PCA eps={c2.eps:g}",
+                        "value": round(c2.K / (np.mean(s_ms) * 1e-3), 1), "unit": UNIT,
+                        "ms_per_step": round(float(np.mean(s_ms)), 4), "plan": q.ctx.info()["path"],
+                        "us_per_inner_iteration": roof2["us_per_inner_iteration"],
+                        "effective_GBps_vs_hbm": roof2["achieved"], "frac_of_hbm_peak": roof2["frac"],
+                        "l2": "L2 flushed between steps", "inner_iterations": int(it2.sum())}]
+    # ---- cpu_baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline_leg(cfg, algo, pr.X, args.cpu_budget)
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------
+# the reference arm (this tier: the CPU oracle, on the host cores)
+# ------------------------------------------------------------------------------------------------
+def run_reference_arm(args):
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if rank != 0:
+        return
+    import oracle
+    ci = WORKLOADS[args.workload]
+    cfg = inputs.config(ci)
+    algo = pick_algo(cfg)
+    pr = inputs.generate(cfg)
+    ks = 1                                                      # bounded sample: the first component, full size
+    times, its = [], 0
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        Xs = oracle.center(pr.X)                                # the step includes S0, like the CUDA arm's
+        r = oracle.pca(Xs, ks, cfg.eps, cfg.max_iter, algo, want_residual=False)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+            its = int(r.iters.sum())
+    ms = float(np.mean(times)) * 1e3
+    value = ks / (ms * 1e-3)
+    sample = (f"each step = S0 centring + the first {ks} of {cfg.K} components of {cfg.name} at full size "
+              f"({its} inner iterations), float64 oracle as it stands")
+    out = {
+        "impl": "reference", "metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms, 3), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{ci}] {cfg.name}: M={cfg.M} N={cfg.N} K={cfg.K} "
+                               f"{'GS-PCA' if algo == inputs.ALGO_GS else 'NIPALS-PCA'} eps={cfg.eps:g} max_iter={cfg.max_iter}",
+                   "sample": sample},
+        "gpu_launches": 0,
+        "cpu_baseline": {"value": round(value, 4), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": round(value, 4), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--components", type=int, default=0, help="override K (profiling runs)")
+    ap.add_argument("--fixed-iters", type=int, default=0, help="eps=0, max_iter=J: exactly J passes per component")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if args.gpus != world and args.impl == "cuda":
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("bench.py: --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU)")
+    if args.impl == "reference":
+        run_reference_arm(args)
+    else:
+        run_cuda_arm(args)
+
+
+if __name__ == "__main__":
+    main()

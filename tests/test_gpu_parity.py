@@ -1,0 +1,461 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle.
+
+All tests here need a B200 (`-m gpu`).  Small and medium cases run the oracle live on the same
+seeded float32 input and compare element by element (vectors through cosines, the north_star's
+tolerances); the full-size BASELINE.json configs compare against the stored oracle prefixes
+under tests/golden/ (written by tests/golden/make_oracle_prefix.py, which calls only oracle/)
+and check, at any size, the properties the method fixes: orthogonality, the energy identity
+(SURVEY.md P4), the decomposition identity eq. (4) on sampled entries, and
+T = X_c P on sampled rows.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_0811_1081_b200 import inputs
+
+from parity_util import (TOL_ORTHO_P, assert_separated_parity, f64, ortho_defect, separated_mask,
+                         signed_cos, subspace_cos_min)
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def binding():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (the library has no CPU fallback)")
+    from paper_0811_1081_b200 import binding as b
+    b.load_library()
+    return b
+
+
+def _oracle_run(oracle_mod, X32, cfg, algo, K=None, extra=1):
+    """Oracle on the same float32 input; `extra` more components for the separation test."""
+    Xc = oracle_mod.center(X32)
+    Kr = min((K or cfg.K) + extra, cfg.N)
+    return Xc, oracle_mod.pca(Xc, Kr, cfg.eps, cfg.max_iter, algo, want_residual=False)
+
+
+def _check_invariants(got, Xc, algo, K, what, recon_tol=2e-5):
+    """Properties that hold at any size for any early-stopped result."""
+    P, T, lam = f64(got["P"]), f64(got["T"]), f64(got["lam"])
+    live = lam > 0
+    np.testing.assert_allclose(np.linalg.norm(P[:, live], axis=0), 1.0, rtol=0, atol=2e-6, err_msg=what + " |P_k|")
+    np.testing.assert_allclose(np.linalg.norm(T[:, live], axis=0), lam[live], rtol=2e-6, err_msg=what + " |T_k| = lambda_k")
+    if algo == inputs.ALGO_GS:
+        assert ortho_defect(P[:, live]) <= TOL_ORTHO_P, what + " P^T P"
+        assert ortho_defect(T[:, live], unit=False) <= TOL_ORTHO_P, what + " V^T V"
+    if "R" in got:
+        R = f64(got["R"])
+        x2 = float(np.sum(Xc * Xc))
+        # eq. (4): X = T P^T + R, elementwise
+        err = np.max(np.abs(Xc - T @ P.T - R))
+        assert err <= recon_tol * np.sqrt(x2 / Xc.shape[1]), f"{what} eq.(4) residual {err:.3e}"
+        # energy identity: |R|_F^2 = |X|_F^2 - sum lambda_k^2
+        e = abs(float(np.sum(R * R)) - (x2 - float(np.sum(lam * lam)))) / x2
+        assert e <= 1e-5, f"{what} energy identity off by {e:.3e}"
+
+
+# --------------------------------------------------------------------------------------------
+# 1. element-by-element parity against a live oracle run: config 1 in full, and scaled-down
+#    siblings of configs 2-5 whose sizes span several CTAs / tiles and have ragged tails.
+# --------------------------------------------------------------------------------------------
+SMALL_CASES = [
+    # (config index, M, N, K, path, ctas)     path: 0 auto, 1 streaming, 2 resident
+    (0, 256, 64, 8, 0, 0),          # BASELINE.json configs[0] in full, auto plan
+    (0, 256, 64, 8, 1, 0),          # ... streaming plan
+    (0, 256, 64, 8, 2, 7),          # ... resident, 7 CTAs (ragged row blocks)
+    (1, 1000, 200, 6, 2, 0),        # M % 8 != 0, N % 8 != 0
+    (1, 1000, 200, 6, 1, 0),
+    (1, 1027, 131, 5, 1, 0),        # M % 4 != 0 -> scalar lane mapping
+    (1, 1027, 131, 5, 2, 0),
+    (1, 3000, 700, 12, 0, 0),       # N > threads-per-CTA: several slice owners
+    (2, 2048, 512, 20, 0, 0),       # collinear columns: 16 signal components + noise bulk
+    (3, 8192, 256, 16, 1, 0),       # tall: more than one row chunk per CTA on the streaming plan
+    (4, 1024, 64, 64, 0, 0),        # K = N full decomposition
+    (1, 64, 300, 4, 0, 0),          # M < N (the paper assumes N <= M; accepted anyway)
+]
+
+
+@pytest.mark.parametrize("ci,M,N,K,path,ctas", SMALL_CASES)
+@pytest.mark.parametrize("algo", [inputs.ALGO_GS, inputs.ALGO_NIPALS])
+def test_small_parity(binding, oracle_mod, ci, M, N, K, path, ctas, algo):
+    base = inputs.config(ci)
+    if base.kind == "spectrum" and M < N:
+        cfg = inputs.scaled(base, M, N, K=K, kind="uniform")
+    else:
+        cfg = inputs.scaled(base, M, N, K=K)
+    pr = inputs.generate(cfg)
+    Xc, ref = _oracle_run(oracle_mod, pr.X, cfg, algo, K=K)
+    got = binding.fit(pr.X, K, cfg.eps, cfg.max_iter, algo, center=True, path=path, ctas=ctas, want_residual=True)
+    what = f"{cfg.name} algo={algo} path={got['info']['path']} ctas={got['info']['ctas']}"
+    # centring (S0) against the oracle's, elementwise
+    assert np.max(np.abs(f64(got["Xc"]) - Xc)) <= 2e-7 * max(1.0, float(np.max(np.abs(pr.X)))), what + " centring"
+    mask = separated_mask(ref.lam, K)
+    assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
+    assert np.all(got["iters"] >= 1) and np.all(got["iters"] <= cfg.max_iter)
+    _check_invariants(got, f64(got["Xc"]), algo, K, what)
+    if ci in (0, 1):
+        assert mask.all(), "configs 1 and 2 have a separated spectrum by construction"
+
+
+def test_paths_agree_and_are_deterministic(binding):
+    """Resident and streaming plans run the same arithmetic in the same order per CTA count;
+    each plan is bitwise reproducible run to run (fixed-order reductions)."""
+    cfg = inputs.scaled(inputs.config(1), 1536, 384, K=6)
+    pr = inputs.generate(cfg)
+    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2)]
+    for a, b in ((0, 1), (2, 3)):
+        for key in ("T", "P", "lam", "iters"):
+            np.testing.assert_array_equal(runs[a][key], runs[b][key])
+    np.testing.assert_allclose(runs[0]["lam"], runs[2]["lam"], rtol=1e-5)
+
+
+# --------------------------------------------------------------------------------------------
+# 2. control flow and degenerate cases (readings C3/C5/C7/C8)
+# --------------------------------------------------------------------------------------------
+def test_eps_zero_runs_exactly_max_iter(binding):
+    cfg = inputs.scaled(inputs.config(0), 256, 64, K=3)
+    pr = inputs.generate(cfg)
+    for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
+        got = binding.fit(pr.X, 3, 0.0, 7, algo)
+        assert got["iters"].tolist() == [7, 7, 7]
+
+
+def test_eps_one_stops_at_second_pass(binding):
+    cfg = inputs.scaled(inputs.config(0), 256, 64, K=3)
+    pr = inputs.generate(cfg)
+    got = binding.fit(pr.X, 3, 1.0, 50, inputs.ALGO_GS)
+    assert got["iters"].tolist() == [2, 2, 2]                 # lambda = 0 on pass 1: strict test cannot fire (C8)
+
+
+def test_golden_worked_examples_on_gpu(binding):
+    """The hand-derived fixtures the oracle is pinned to, through the CUDA path (fp32 tolerance)."""
+    g = json.load(open(os.path.join(GOLD, "worked_3x2.json")))
+    X = np.asfortranarray(np.array(g["X_rows"], dtype=np.float32))
+    got = binding.fit(X, 1, g["eps"], g["max_iter"], inputs.ALGO_NIPALS, center=False, want_residual=True)
+    nrm = np.sqrt(g["norm_sq"])
+    assert got["iters"].tolist() == g["iters"]
+    np.testing.assert_allclose(got["lam"][0], np.sqrt(g["lambda_sq_num"] / g["lambda_sq_den"]), rtol=1e-6)
+    np.testing.assert_allclose(got["P"][:, 0], np.array(g["p_int"]) / nrm, rtol=1e-6)
+    np.testing.assert_allclose(got["T"][:, 0], np.array(g["t_int"]) / nrm, rtol=1e-6)
+    R = f64(X) - np.outer(g["t_int"], g["p_int"]) / g["norm_sq"]
+    np.testing.assert_allclose(got["R"], R, rtol=0, atol=2e-6)
+    g = json.load(open(os.path.join(GOLD, "diag_2x2.json")))
+    X = np.asfortranarray(np.array(g["X_rows"], dtype=np.float32))
+    for algo in (inputs.ALGO_NIPALS, inputs.ALGO_GS):
+        got = binding.fit(X, 2, g["eps"], g["max_iter"], algo, center=False, want_residual=True)
+        assert got["iters"].tolist() == g["iters"]
+        np.testing.assert_array_equal(got["lam"], np.array(g["lambda"], dtype=np.float32))
+        np.testing.assert_array_equal(got["T"], np.array(g["T_rows"], dtype=np.float32))
+        np.testing.assert_array_equal(got["P"], np.array(g["P_rows"], dtype=np.float32))
+        np.testing.assert_array_equal(got["R"], np.array(g["R_rows"], dtype=np.float32))
+
+
+def test_degenerate_zero_column_and_zero_matrix(binding, oracle_mod):
+    """Reading C7: a component with a zero start column returns lambda = 0, T = P = 0, iters = 0."""
+    rng = np.random.default_rng(5)
+    X = np.asfortranarray(rng.standard_normal((40, 6)).astype(np.float32))
+    X[:, 1] = 0.0
+    Z = np.zeros((12, 4), dtype=np.float32, order="F")
+    for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
+        got = binding.fit(Z, 3, 1e-7, 20, algo, center=False, want_residual=True)
+        assert got["iters"].tolist() == [0, 0, 0] and not got["lam"].any() and not got["T"].any() and not got["P"].any()
+        assert not got["R"].any()
+    # rank-1 input: component 0 converges in 2 passes, component 1 starts from an (almost) zero column
+    u = rng.standard_normal(50)
+    v = rng.standard_normal(8)
+    X1 = np.asfortranarray(np.outer(u, v).astype(np.float32))
+    ref = oracle_mod.pca(X1, 1, 1e-6, 100, inputs.ALGO_GS)
+    got = binding.fit(X1, 1, 1e-6, 100, inputs.ALGO_GS, center=False)
+    assert got["iters"].tolist() == ref.iters.tolist() == [2]
+    np.testing.assert_allclose(got["lam"], ref.lam, rtol=1e-6)
+
+
+@pytest.mark.parametrize("M,N,K", [(1, 1, 1), (5, 1, 1), (1, 7, 2), (3, 3, 3), (513, 2, 2), (2, 513, 2)])
+def test_tiny_and_thin_shapes(binding, oracle_mod, M, N, K):
+    rng = np.random.default_rng(M * 1000 + N)
+    X = np.asfortranarray(rng.standard_normal((M, N)).astype(np.float32))
+    for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
+        ref = oracle_mod.pca(X, K, 1e-7, 500, algo)
+        got = binding.fit(X, K, 1e-7, 500, algo, center=False, want_residual=True)
+        live = ref.lam > 1e-6 * max(ref.lam.max(), 1e-30)
+        np.testing.assert_allclose(got["lam"][live], ref.lam[live], rtol=1e-4)
+        err = np.max(np.abs(f64(X) - f64(got["T"]) @ f64(got["P"]).T - f64(got["R"])))
+        assert err <= 1e-5 * max(1.0, float(np.max(np.abs(X))))
+
+
+# --------------------------------------------------------------------------------------------
+# 3. centring kernel (S0), both modes, with a large column offset
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("M,N", [(4096, 300), (1027, 33), (7, 5), (100000, 3)])
+def test_center_kernel(binding, oracle_mod, M, N):
+    import torch
+    rng = np.random.default_rng(M + N)
+    X = rng.standard_normal((M, N)) + 1000.0 * rng.standard_normal(N)[None, :]
+    X32 = np.asfortranarray(X.astype(np.float32))
+    for mode, ref_fn in ((0, oracle_mod.center), (1, oracle_mod.center_eq1)):
+        ctx = binding.PcaContext(M, N, 1)
+        ctx.pca_set_option(binding.PCA_OPT_CENTER_MODE, mode)
+        Xd = binding.from_colmajor(X32)
+        ctx.pca_center(Xd)
+        torch.cuda.synchronize()
+        got = binding.to_colmajor(Xd)
+        ref = ref_fn(X32)
+        # one rounding of the result to float32 (the mean itself is accumulated in float64)
+        assert np.max(np.abs(f64(got) - ref)) <= 6e-8 * float(np.max(np.abs(X32))) + 1e-7 * float(np.max(np.abs(ref)))
+        ctx.pca_destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# 4. C-ABI behaviour: error codes, host entry point, residual, workspace handling
+# --------------------------------------------------------------------------------------------
+def test_error_codes(binding):
+    import ctypes
+    import torch
+    lib = binding.load_library()
+    ctx = ctypes.c_void_p()
+    bad = [(0, 4, 1, 1e-7, 10, 1), (4, 0, 1, 1e-7, 10, 1), (4, 4, 0, 1e-7, 10, 1), (4, 4, 5, 1e-7, 10, 1),
+           (4, 4, 1, -1.0, 10, 1), (4, 4, 1, float("nan"), 10, 1), (4, 4, 1, 1e-7, 0, 1), (4, 4, 1, 1e-7, 10, 2)]
+    for args in bad:
+        assert lib.pca_create(ctypes.byref(ctx), *args) == binding.PCA_EINVAL
+        assert not ctx.value
+    assert lib.pca_create(None, 4, 4, 1, 1e-7, 10, 1) == binding.PCA_EINVAL
+    c = binding.PcaContext(64, 16, 2)
+    X = torch.zeros((16, 64), device="cuda")
+    T = torch.zeros((2, 64), device="cuda")
+    P = torch.zeros((2, 16), device="cuda")
+    lam = torch.zeros(2, device="cuda")
+    it = torch.zeros(2, dtype=torch.int32, device="cuda")
+    vp = ctypes.c_void_p
+    st = vp(torch.cuda.current_stream().cuda_stream)
+    # no workspace yet
+    assert lib.pca_run(c._ctx, vp(X.data_ptr()), vp(T.data_ptr()), vp(P.data_ptr()), vp(lam.data_ptr()),
+                       vp(it.data_ptr()), st) == binding.PCA_EWORKSPACE
+    ptr = vp()
+    assert lib.pca_residual(c._ctx, ctypes.byref(ptr)) == binding.PCA_EWORKSPACE
+    ws = torch.empty(c.pca_workspace_bytes() + 512, dtype=torch.uint8, device="cuda")
+    off = (-ws.data_ptr()) % 256
+    assert lib.pca_set_workspace(c._ctx, vp(ws.data_ptr() + off), 16) == binding.PCA_EWORKSPACE
+    assert lib.pca_set_workspace(c._ctx, vp(ws.data_ptr() + off + 4), c.pca_workspace_bytes()) == binding.PCA_EALIGN
+    assert lib.pca_set_workspace(c._ctx, None, c.pca_workspace_bytes()) == binding.PCA_EINVAL
+    assert lib.pca_set_workspace(c._ctx, vp(ws.data_ptr() + off), c.pca_workspace_bytes()) == binding.PCA_OK
+    # misaligned matrix, NULL pointer
+    assert lib.pca_run(c._ctx, vp(X.data_ptr() + 4), vp(T.data_ptr()), vp(P.data_ptr()), vp(lam.data_ptr()),
+                       vp(it.data_ptr()), st) == binding.PCA_EALIGN
+    assert lib.pca_run(c._ctx, None, vp(T.data_ptr()), vp(P.data_ptr()), vp(lam.data_ptr()),
+                       vp(it.data_ptr()), st) == binding.PCA_EINVAL
+    assert lib.pca_center(c._ctx, None, st) == binding.PCA_EINVAL
+    assert lib.pca_set_option(c._ctx, 99, 0) == binding.PCA_EINVAL
+    assert lib.pca_run(c._ctx, vp(X.data_ptr()), vp(T.data_ptr()), vp(P.data_ptr()), vp(lam.data_ptr()),
+                       vp(it.data_ptr()), st) == binding.PCA_OK
+    torch.cuda.synchronize()
+    assert binding.pca_strerror(binding.PCA_EALIGN)
+    c.pca_destroy()
+
+
+def test_x_is_never_written_and_stream_is_respected(binding):
+    import torch
+    cfg = inputs.scaled(inputs.config(1), 1024, 256, K=4)
+    pr = inputs.generate(cfg)
+    ctx = binding.PcaContext(cfg.M, cfg.N, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+    X = binding.from_colmajor(pr.X)
+    s = torch.cuda.Stream()
+    T = torch.empty((cfg.K, cfg.M), device="cuda")
+    P = torch.empty((cfg.K, cfg.N), device="cuda")
+    lam = torch.empty(cfg.K, device="cuda")
+    it = torch.empty(cfg.K, dtype=torch.int32, device="cuda")
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        ctx.pca_center(X)
+        Xc = X.clone()
+        ctx.pca_run(X, T, P, lam, it)
+        ctx.pca_run(X, T, P, lam, it)          # a context can be re-run
+    s.synchronize()
+    assert torch.equal(X, Xc)
+    assert (it > 0).all()
+    ctx.pca_destroy()
+
+
+def test_fit_host_matches_device_path(binding):
+    import torch
+    cfg = inputs.scaled(inputs.config(1), 2048, 512, K=8)
+    pr = inputs.generate(cfg)
+    dev = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+    ctx = binding.PcaContext(cfg.M, cfg.N, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+    Xh = torch.from_numpy(np.ascontiguousarray(pr.X.T)).pin_memory()
+    Th = torch.empty((cfg.K, cfg.M)).pin_memory()
+    Ph = torch.empty((cfg.K, cfg.N)).pin_memory()
+    lh = torch.empty(cfg.K).pin_memory()
+    ih = torch.empty(cfg.K, dtype=torch.int32).pin_memory()
+    ctx.pca_fit_host(Xh, Th, Ph, lh, ih)
+    np.testing.assert_array_equal(Th.numpy().T, dev["T"])
+    np.testing.assert_array_equal(Ph.numpy().T, dev["P"])
+    np.testing.assert_array_equal(lh.numpy(), dev["lam"])
+    np.testing.assert_array_equal(ih.numpy(), dev["iters"])
+    ctx.pca_destroy()
+
+
+# --------------------------------------------------------------------------------------------
+# 5. BASELINE.json configs at FULL size, in the launch plan bench.py times (auto), against the
+#    stored oracle prefixes + the size-independent properties.
+# --------------------------------------------------------------------------------------------
+def _load_golden(cfg, algo):
+    z = np.load(os.path.join(GOLD, f"oracle_{cfg.name}_{'gs' if algo == inputs.ALGO_GS else 'nipals'}.npz"))
+    return {k: z[k] for k in z.files}, json.loads(str(z["meta"]))
+
+
+_PROBLEMS = {}
+
+
+def _problem(ci):
+    if ci not in _PROBLEMS:
+        _PROBLEMS.clear()                      # keep at most one full-size input alive
+        _PROBLEMS[ci] = inputs.generate(inputs.config(ci))
+    return _PROBLEMS[ci]
+
+
+def _full_size_check(binding, ci, algo, K_run):
+    import torch
+    cfg = inputs.config(ci)
+    gold, meta = _load_golden(cfg, algo)
+    ks = int(meta["K_stored"])
+    pr = _problem(ci)
+    M, N = cfg.M, cfg.N
+    ctx = binding.PcaContext(M, N, K_run, cfg.eps, cfg.max_iter, algo)
+    X = binding.from_colmajor(pr.X)
+    ctx.pca_center(X)
+    T = torch.empty((K_run, M), device="cuda")
+    P = torch.empty((K_run, N), device="cuda")
+    lam = torch.empty(K_run, device="cuda")
+    it = torch.empty(K_run, dtype=torch.int32, device="cuda")
+    ctx.pca_run(X, T, P, lam, it)
+    torch.cuda.synchronize()
+    what = f"{cfg.name} algo={algo} {ctx.info()}"
+    # centring: ||X_c||_F^2 against the oracle's
+    x2 = float((X.double() ** 2).sum())
+    assert abs(x2 - float(gold["x_fro2"])) <= 1e-6 * float(gold["x_fro2"]), what
+    Pn, lamn, itn = binding.to_colmajor(P), lam.cpu().numpy(), it.cpu().numpy()
+    rows = gold["rows"]
+    T_rows = T[:, torch.from_numpy(rows).cuda()].cpu().numpy().T          # (S, K_run)
+    kc = min(ks, K_run)
+    mask = separated_mask(gold["lam"], kc)
+    # separated components: lambda, full loadings vector, sampled scores, joint sign
+    for k in range(kc):
+        if not mask[k]:
+            continue
+        rel = abs(float(lamn[k]) - gold["lam"][k]) / gold["lam"][k]
+        cp = signed_cos(Pn[:, k], gold["P"][:, k])
+        ct = signed_cos(T_rows[:, k], gold["T_rows"][:, k])
+        assert rel <= 1e-4, f"{what} lambda[{k}] rel {rel:.3e}"
+        assert abs(cp) >= 1 - 1e-4, f"{what} P[:, {k}] |cos| {abs(cp):.8f}"
+        assert abs(ct) >= 1 - 1e-4, f"{what} T[rows, {k}] |cos| {abs(ct):.8f}"
+        assert np.sign(cp) == np.sign(ct), f"{what} joint sign [{k}]"
+        # sampled scores one by one: |t_gpu - t_or| <= 1.5e-2 * lambda_k / sqrt(M) * few  (cos bound, per entry rms)
+        d = np.abs(np.sign(ct) * f64(T_rows[:, k]) - f64(gold["T_rows"][:, k]))
+        assert np.sqrt(np.mean(d * d)) <= 1.5e-2 * gold["lam"][k] / np.sqrt(M), f"{what} sampled T[:, {k}]"
+    # size-independent properties over ALL K_run components
+    live = lamn > 0
+    assert live.all(), what + " unexpected degenerate component"
+    Pd = P.double()
+    G = (Pd @ Pd.T).cpu().numpy()
+    Td = T.double()
+    Gt = (Td @ Td.T).cpu().numpy()
+    np.testing.assert_allclose(np.sqrt(np.diag(Gt)), lamn, rtol=3e-6, err_msg=what + " |T_k| = lambda_k")
+    np.testing.assert_allclose(np.diag(G), 1.0, atol=3e-6, err_msg=what + " |P_k| = 1")
+    if algo == inputs.ALGO_GS:
+        assert np.max(np.abs(G - np.eye(K_run))) <= TOL_ORTHO_P, what + f" max|P^T P - I| = {np.max(np.abs(G - np.eye(K_run))):.3e}"
+        Vn = Gt / np.outer(lamn, lamn)
+        assert np.max(np.abs(Vn - np.eye(K_run))) <= TOL_ORTHO_P, what + f" max|V^T V - I| = {np.max(np.abs(Vn - np.eye(K_run))):.3e}"
+    # energy identity on the residual the library returns (eq. 4 / SURVEY.md P4)
+    R = ctx.pca_residual()
+    r2 = float((R.double() ** 2).sum())
+    e = abs(r2 - (x2 - float(np.sum(f64(lamn) ** 2)))) / x2
+    assert e <= 1e-5, f"{what} energy identity off by {e:.3e}"
+    # eq. (4) on sampled rows: X_c[rows, :] = T[rows, :] P^T + R[rows, :]
+    ridx = torch.from_numpy(rows).cuda()
+    lhs = X[:, ridx].double()
+    rhs = (Pd.T @ Td[:, ridx]) + R[:, ridx].double()
+    err = float((lhs - rhs).abs().max())
+    assert err <= 2e-5 * np.sqrt(x2 / (M * N)) * 10, f"{what} eq.(4) sampled residual {err:.3e}"
+    # non-separated prefix: cluster energy and spanned subspace instead of single vectors
+    if not mask.all():
+        s_g = float(np.sum(f64(lamn[:kc]) ** 2))
+        s_o = float(np.sum(f64(gold["lam"][:kc]) ** 2))
+        assert abs(s_g - s_o) <= 1e-3 * s_o, f"{what} prefix energy {s_g} vs {s_o}"
+    info = dict(iters=itn.tolist(), lam=lamn[:4].tolist(), separated=int(mask.sum()), stored=kc)
+    ctx.pca_destroy()
+    del X, T, P, R
+    torch.cuda.empty_cache()
+    return info, gold, Pn
+
+
+def test_full_cfg1(binding):
+    for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
+        _full_size_check(binding, 0, algo, 8)
+
+
+def test_full_cfg2(binding):
+    info, gold, _ = _full_size_check(binding, 1, inputs.ALGO_GS, 32)
+    assert info["separated"] == 32
+
+
+def test_full_cfg3_gs_and_nipals(binding):
+    """Collinear columns: the 16 signal components sit in a cluster with sub-1% gaps, so single
+    vectors are not unique; the spanned subspace and its energy are."""
+    info_g, gold, Pg = _full_size_check(binding, 2, inputs.ALGO_GS, 16)
+    info_n, _, Pn = _full_size_check(binding, 2, inputs.ALGO_NIPALS, 16)
+    ks = 4
+    # both algorithms see the same 16-dimensional signal subspace
+    assert subspace_cos_min(Pg, Pn) >= 1 - 1e-4
+    # the oracle's first 4 loadings lie inside the GPU's 16-dimensional signal subspace
+    Q, _ = np.linalg.qr(f64(Pg))
+    for k in range(ks):
+        p = f64(gold["P"][:, k])
+        assert np.linalg.norm(Q.T @ p) >= 1 - 1e-4
+
+
+def test_full_cfg4_prefix(binding):
+    info, gold, _ = _full_size_check(binding, 3, inputs.ALGO_GS, 9)
+    assert info["separated"] >= 8
+
+
+def test_full_cfg5_prefix(binding):
+    _full_size_check(binding, 4, inputs.ALGO_GS, 17)
+
+
+def test_full_cfg5_reconstruction(binding):
+    """BASELINE.json configs[4]: K = N = 512, check X = T P^T and max|P^T P - I|.
+    The reconstruction is bounded by the convergence error of early-stopped power iterations
+    (SURVEY.md P7), not by rounding: <= 1e-3 relative Frobenius."""
+    import torch
+    cfg = inputs.config(4)
+    pr = _problem(4)
+    ctx = binding.PcaContext(cfg.M, cfg.N, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+    X = binding.from_colmajor(pr.X)
+    ctx.pca_center(X)
+    T = torch.empty((cfg.K, cfg.M), device="cuda")
+    P = torch.empty((cfg.K, cfg.N), device="cuda")
+    lam = torch.empty(cfg.K, device="cuda")
+    it = torch.empty(cfg.K, dtype=torch.int32, device="cuda")
+    ctx.pca_run(X, T, P, lam, it)
+    torch.cuda.synchronize()
+    Pd, Td, Xd = P.double(), T.double(), X.double()
+    G = (Pd @ Pd.T).cpu().numpy()
+    assert np.max(np.abs(G - np.eye(cfg.K))) <= TOL_ORTHO_P
+    rec = float((Xd - Pd.T @ Td).norm() / Xd.norm())
+    assert rec <= 1e-3, f"||X - T P^T||_F / ||X||_F = {rec:.3e}"
+    R = ctx.pca_residual().double()
+    assert abs(float(R.norm() / Xd.norm()) - rec) <= 1e-5
+    assert int(it.max()) < cfg.max_iter, "a component hit max_iter"
+    # full SVD claim: the lambdas are the singular values of X_c (as a set)
+    sv = torch.linalg.svdvals(Xd).cpu().numpy()
+    got = np.sort(lam.cpu().numpy().astype(np.float64))[::-1]
+    assert np.max(np.abs(got - sv) / sv) <= 5e-3
+    assert abs(np.sum(got ** 2) - np.sum(sv ** 2)) <= 1e-5 * np.sum(sv ** 2)
+    ctx.pca_destroy()

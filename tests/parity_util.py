@@ -7,8 +7,14 @@ matrices) in float64 numpy.  Tolerances are BASELINE.json's north_star values:
     GS-PCA               :  max |P^T P - I| <= 1e-5
 "separated" is decided from the ORACLE's lambdas only (reading P9):
 component k is separated when every other stored oracle lambda differs from lambda_k by at
-least 1 % of lambda_k.  Non-separated components have no unique early-stopped vector
-(several results are correct); for them the tests check what is unique: invariants.
+least 2 % of lambda_k.  Why 2 %: the method stops early, so even the float64 oracle's vector is
+off the true singular vector by 1 - cos ~= 0.15 * eps / gap^2 (measured oracle-vs-SVD on the
+scaled config 3: 1.1e-4 at a 1.2 % gap, 2.7e-5 at 2.9 %, 8e-6 at 3.3 %, eps = 1e-7); which
+early-stopped vector comes out depends on the pass at which the stagnation test fires, and that
+legitimately differs between float32 and float64 (reading C4).  Below a 2 % gap this ambiguity
+alone reaches the 1e-4 tolerance, so single vectors are not a unique result there.
+Non-separated components have no unique early-stopped vector (several results are correct);
+for them the tests check what is unique: invariants, cluster energy, spanned subspace.
 """
 from __future__ import annotations
 
@@ -17,7 +23,7 @@ import numpy as np
 TOL_LAMBDA = 1e-4
 TOL_COS = 1e-4
 TOL_ORTHO_P = 1e-5
-SEPARATION = 1e-2
+SEPARATION = 2e-2
 
 
 def f64(a):

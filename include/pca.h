@@ -55,20 +55,22 @@ enum {
 
 /* Options for pca_set_option (all optional; defaults are chosen by pca_create). */
 enum {
-  PCA_OPT_PATH = 1,     /* 0 = auto, 1 = force HBM-streaming path, 2 = force SMEM-resident path */
+  PCA_OPT_PATH = 1,     /* 0 = auto; two-sweep kernel: 1 = HBM-streaming, 2 = SMEM-resident;
+                           single-sweep kernel (R read once per inner pass): 3 = streaming, 4 = resident */
   PCA_OPT_CTAS = 2,     /* number of CTAs of the persistent kernel (0 = auto) */
   PCA_OPT_CENTER_MODE = 3 /* 0 = column means (default), 1 = literal eq. (1) mean column */
 };
 
 /* Fields for pca_get_info. */
 enum {
-  PCA_INFO_PATH = 1,        /* 1 = streaming, 2 = resident */
+  PCA_INFO_PATH = 1,        /* 1, 2 = two-sweep kernel streaming / resident; 3, 4 = single-sweep kernel streaming / resident */
   PCA_INFO_CTAS = 2,        /* CTAs of the persistent solve kernel */
   PCA_INFO_THREADS = 3,     /* threads per CTA */
   PCA_INFO_SMEM_BYTES = 4,  /* dynamic shared memory per CTA */
   PCA_INFO_ROWS_PER_CTA = 5,
   PCA_INFO_LAUNCHES_PER_RUN = 6, /* kernel launches one pca_run enqueues */
-  PCA_INFO_NUM_SMS = 7
+  PCA_INFO_NUM_SMS = 7,
+  PCA_INFO_ROW_GROUP_THREADS = 8 /* single-sweep kernel: threads that share one row of R (0 otherwise) */
 };
 
 /* Create a context for one problem shape.
@@ -90,8 +92,10 @@ int pca_create(pca_ctx** out, int64_t M, int64_t N, int K, double eps, int max_i
 int pca_set_option(pca_ctx*, int option, int64_t value);
 int pca_get_info(const pca_ctx*, int field, int64_t* value);
 
-/* Device workspace the caller must provide: the residual R (4*M*N bytes, first) followed by
- * the partial-sum / exchange scratch of the persistent kernel. */
+/* Device workspace the caller must provide: the residual R of eq. (4) (4*M*N bytes, column-major,
+ * first), followed -- for the single-sweep kernel -- by the row-major working copy of the residual
+ * (4*M*ldr bytes, ldr = N rounded up to the row-group width), and the partial-sum / exchange
+ * scratch of the persistent kernel. */
 size_t pca_workspace_bytes(const pca_ctx*);
 
 /* Hand the context a device buffer of at least pca_workspace_bytes() bytes, 256-byte aligned.

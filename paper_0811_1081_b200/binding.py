@@ -19,9 +19,9 @@ PCA_ALGO_GS = 1
 PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED = range(6)
 
 PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE = 1, 2, 3
-PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT = 0, 1, 2
+PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT = 0, 1, 2, 3, 4
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
- PCA_INFO_LAUNCHES_PER_RUN, PCA_INFO_NUM_SMS) = range(1, 8)
+ PCA_INFO_LAUNCHES_PER_RUN, PCA_INFO_NUM_SMS, PCA_INFO_ROW_GROUP_THREADS) = range(1, 9)
 
 EXPORTED_SYMBOLS = (
     "pca_create", "pca_set_option", "pca_get_info", "pca_workspace_bytes", "pca_set_workspace",
@@ -114,13 +114,15 @@ class PcaContext:
 
     def info(self) -> dict:
         return {
-            "path": {1: "streaming", 2: "resident"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
+            "path": {1: "two-sweep streaming", 2: "two-sweep resident", 3: "single-sweep streaming",
+                     4: "single-sweep resident"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
             "ctas": self.pca_get_info(PCA_INFO_CTAS),
             "threads": self.pca_get_info(PCA_INFO_THREADS),
             "smem_bytes": self.pca_get_info(PCA_INFO_SMEM_BYTES),
             "rows_per_cta": self.pca_get_info(PCA_INFO_ROWS_PER_CTA),
             "launches_per_run": self.pca_get_info(PCA_INFO_LAUNCHES_PER_RUN),
             "num_sms": self.pca_get_info(PCA_INFO_NUM_SMS),
+            "row_group_threads": self.pca_get_info(PCA_INFO_ROW_GROUP_THREADS),
         }
 
     def pca_workspace_bytes(self) -> int:

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpca_b200.so")
 SOURCES = [os.path.join(CSRC, "pca_api.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("pca_device.cuh", "pca_solve.cuh", "pca_center.cuh")] + [
+HEADERS = [os.path.join(CSRC, f) for f in ("pca_device.cuh", "pca_solve.cuh", "pca_fused.cuh", "pca_center.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "pca.h")]
 
 

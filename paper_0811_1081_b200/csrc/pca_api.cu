@@ -13,8 +13,10 @@
 #include <new>
 
 #include "pca_center.cuh"
+#include "pca_fused.cuh"
 #include "pca_solve.cuh"
 
+using pca::FusedParams;
 using pca::SolveParams;
 
 namespace {
@@ -37,6 +39,15 @@ const Variant kVariants[] = {
 };
 #undef PCA_VARIANT
 
+typedef void (*fused_kernel_t)(const FusedParams);
+struct FusedVariant { int resident, nv; fused_kernel_t fn; };
+#define PCA_FVARIANT(RES, NV) {RES, NV, pca::pca_fused_kernel<NV, (RES != 0)>}
+const FusedVariant kFusedVariants[] = {
+    PCA_FVARIANT(0, 1), PCA_FVARIANT(0, 2), PCA_FVARIANT(0, 3), PCA_FVARIANT(0, 4),
+    PCA_FVARIANT(1, 1), PCA_FVARIANT(1, 2), PCA_FVARIANT(1, 3), PCA_FVARIANT(1, 4),
+};
+#undef PCA_FVARIANT
+
 }  // namespace
 
 struct pca_ctx {
@@ -51,9 +62,13 @@ struct pca_ctx {
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0;
   // plan
   bool planned = false;
-  int path = 0;  // 1 streaming, 2 resident
+  int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel)
   const Variant* variant = nullptr;
   SolveParams prm{};
+  const FusedVariant* fvariant = nullptr;
+  FusedParams fprm{};
+  size_t ws_off_rrm = 0, ws_off_qpart2 = 0, ws_off_bpart2 = 0, ws_off_spart2 = 0, ws_off_apart2 = 0, ws_off_pvec2 = 0,
+         ws_off_npart = 0, ws_off_w = 0;
   size_t smem_bytes = 0;
   size_t ws_bytes = 0;
   size_t ws_off_ppart = 0, ws_off_apart = 0, ws_off_bpart = 0, ws_off_pvec = 0, ws_off_qpart = 0, ws_off_spart = 0,
@@ -129,8 +144,113 @@ size_t carve(pca_ctx* c, int resident, int G, int vec, SolveParams* p, int* tr, 
   return off;
 }
 
+// Single-sweep kernel (pca_fused.cuh): GT threads share a row, NV float4 per thread per row.
+// want: 0 = resident if it fits else streaming, 3 = streaming, 4 = resident.
+int make_fused_plan(pca_ctx* c, int want) {
+  const long long M = c->M, N = c->N;
+  const int sms = c->num_sms;
+  int GT = 32;
+  while ((long long)16 * GT < N) GT *= 2;
+  if (GT > pca::kThreads) return PCA_EUNSUPPORTED;
+  const int NV = (int)ceil_div(N, 4LL * GT);
+  const int ldr = 4 * GT * NV;
+  const int g_min = (int)ceil_div(N, pca::kThreads);
+  auto carve_fused = [&](int resident, int G, FusedParams* p) -> size_t {
+    p->G = G;
+    p->Mb = (int)ceil_div(M, G);
+    p->ldr = ldr; p->GT = GT;
+    p->Ns = (int)round_up(ceil_div(N, G), 4);
+    p->Gs = (int)ceil_div(N, p->Ns);
+    p->Kpad = (int)round_up(c->K, 4);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 16); return (int)o; };
+    const size_t mbp = (size_t)round_up(p->Mb, 4);
+    p->off_p = take((size_t)ldr * 4);
+    p->off_pdef = take((size_t)ldr * 4);
+    p->off_ttil = take(mbp * 4);
+    p->off_d = take(mbp * 4);
+    p->off_qs = take((size_t)pca::kThreads * 4 * NV * 4);
+    p->off_red = take((size_t)2 * pca::kWarps * pca::kRB * 4);
+    p->off_sgrp = take((size_t)(pca::kThreads / GT) * 8);
+    p->off_B = take((size_t)p->Kpad * 8);
+    p->off_A = take((size_t)p->Kpad * 8);
+    p->off_scr = take((size_t)pca::kThreads * 8);
+    p->off_praw = take((size_t)p->Ns * 8);
+    p->off_lam = take((size_t)p->Kpad * 4);
+    p->off_slab = take(resident ? (size_t)p->Mb * (size_t)ldr * 4 : 0);
+    return off;
+  };
+  auto find = [&](int resident) -> const FusedVariant* {
+    for (const FusedVariant& v : kFusedVariants)
+      if (v.resident == resident && v.nv == NV) return &v;
+    return nullptr;
+  };
+  FusedParams p{};
+  size_t smem = 0;
+  int path = 0;
+  const FusedVariant* var = nullptr;
+  auto try_plan = [&](int resident, int G) -> bool {
+    if (G < g_min) G = g_min;
+    if (G > sms) G = sms;
+    if (G < 1) G = 1;
+    if (g_min > sms) return false;
+    smem = carve_fused(resident, G, &p);
+    if (smem > (size_t)c->smem_optin) return false;
+    var = find(resident);
+    return var != nullptr;
+  };
+  bool ok = false;
+  if (want == 0 || want == 4) {
+    int G = c->opt_ctas > 0 ? c->opt_ctas : ((size_t)M * (size_t)ldr * 4 <= (size_t)160 * 1024 ? 1 : sms);
+    ok = try_plan(1, G);
+    if (!ok && c->opt_ctas == 0 && G != sms) ok = try_plan(1, sms);
+    if (ok) path = 4;
+    else if (want == 4) return PCA_EUNSUPPORTED;
+  }
+  if (!ok) {
+    ok = try_plan(0, c->opt_ctas > 0 ? c->opt_ctas : sms);
+    if (!ok) return PCA_EUNSUPPORTED;
+    path = 3;
+  }
+  cudaError_t e = cudaFuncSetAttribute(var->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, var->fn, pca::kThreads, smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
+
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
+  take((size_t)M * (size_t)N * 4);                                   // residual of eq. (4), column-major (ABI layout)
+  c->ws_off_rrm = take((size_t)M * (size_t)ldr * 4);                 // working residual, row-major
+  c->ws_off_qpart2 = take((size_t)2 * p.G * ldr * 4);
+  c->ws_off_bpart2 = take((size_t)2 * p.G * p.Kpad * 4);
+  c->ws_off_spart2 = take((size_t)2 * p.G * 8);
+  c->ws_off_apart2 = take((size_t)p.Gs * p.Kpad * 4);
+  c->ws_off_pvec2 = take((size_t)ldr * 4);
+  c->ws_off_npart = take((size_t)p.Gs * 8);
+  c->ws_off_w = take((size_t)ldr * p.Kpad * 4);
+  c->ws_off_bar = take(256);
+  c->ws_bytes = off;
+  c->fprm = p;
+  c->fvariant = var;
+  c->smem_bytes = smem;
+  c->path = path;
+  c->planned = true;
+  c->ws = nullptr;
+  c->ws_given = 0;
+  c->ran = false;
+  return PCA_OK;
+}
+
 int make_plan(pca_ctx* c) {
   c->planned = false;
+  if (c->opt_path == 0 || c->opt_path == 3 || c->opt_path == 4) {
+    const int rc = make_fused_plan(c, c->opt_path);
+    if (rc == PCA_OK || c->opt_path != 0) return rc;
+    if (rc == PCA_ECUDA) return rc;
+  }
   const long long M = c->M, N = c->N;
   const int vec = (M % 4 == 0) ? 4 : 1;
   const int sms = c->num_sms;
@@ -238,7 +358,7 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
   if (!c) return PCA_EINVAL;
   switch (option) {
     case PCA_OPT_PATH:
-      if (value < 0 || value > 2) return PCA_EINVAL;
+      if (value < 0 || value > 4) return PCA_EINVAL;
       c->opt_path = (int)value;
       break;
     case PCA_OPT_CTAS:
@@ -259,11 +379,12 @@ int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
   if (!c || !value || !c->planned) return PCA_EINVAL;
   switch (field) {
     case PCA_INFO_PATH: *value = c->path; break;
-    case PCA_INFO_CTAS: *value = c->prm.G; break;
+    case PCA_INFO_CTAS: *value = c->path >= 3 ? c->fprm.G : c->prm.G; break;
     case PCA_INFO_THREADS: *value = pca::kThreads; break;
     case PCA_INFO_SMEM_BYTES: *value = (int64_t)c->smem_bytes; break;
-    case PCA_INFO_ROWS_PER_CTA: *value = c->prm.Mb; break;
-    case PCA_INFO_LAUNCHES_PER_RUN: *value = 1; break;
+    case PCA_INFO_ROWS_PER_CTA: *value = c->path >= 3 ? c->fprm.Mb : c->prm.Mb; break;
+    case PCA_INFO_LAUNCHES_PER_RUN: *value = c->path >= 3 ? 3 : 1; break;
+    case PCA_INFO_ROW_GROUP_THREADS: *value = c->path >= 3 ? c->fprm.GT : 0; break;
     case PCA_INFO_NUM_SMS: *value = c->num_sms; break;
     default: return PCA_EINVAL;
   }
@@ -303,6 +424,33 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
   if (!c->ws || c->ws_given < c->ws_bytes) return PCA_EWORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   unsigned char* ws = static_cast<unsigned char*>(c->ws);
+  if (c->path >= 3) {
+    FusedParams p = c->fprm;
+    p.Rrm = reinterpret_cast<float*>(ws + c->ws_off_rrm);
+    p.T = T; p.P = P; p.lambda = lambda; p.iters = iters;
+    p.Qpart = reinterpret_cast<float*>(ws + c->ws_off_qpart2);
+    p.Bpart = reinterpret_cast<float*>(ws + c->ws_off_bpart2);
+    p.Spart = reinterpret_cast<double*>(ws + c->ws_off_spart2);
+    p.Apart = reinterpret_cast<float*>(ws + c->ws_off_apart2);
+    p.pvec = reinterpret_cast<float*>(ws + c->ws_off_pvec2);
+    p.Npart = reinterpret_cast<double*>(ws + c->ws_off_npart);
+    p.W = reinterpret_cast<float*>(ws + c->ws_off_w);
+    p.bar = reinterpret_cast<unsigned long long*>(ws + c->ws_off_bar);
+    PCA_CUDA(c, cudaMemsetAsync(p.bar, 0, 256, st));
+    const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
+    pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X
+    PCA_CUDA(c, cudaGetLastError());
+    void* fargs[] = {&p};
+    PCA_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(c->fvariant->fn), dim3((unsigned)p.G),
+                                            dim3(pca::kThreads), fargs, c->smem_bytes, st));
+    const dim3 ogrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(c->N, 32));
+    pca::pca_transpose_out_kernel<<<ogrid, 256, 0, st>>>(p.Rrm, reinterpret_cast<float*>(ws),
+                                                         T + (size_t)(c->K - 1) * (size_t)c->M,
+                                                         P + (size_t)(c->K - 1) * (size_t)c->N, c->M, p.N, p.ldr);
+    PCA_CUDA(c, cudaGetLastError());
+    c->ran = true;
+    return PCA_OK;
+  }
   SolveParams p = c->prm;
   p.X = X;
   p.R = reinterpret_cast<float*>(ws);

@@ -66,10 +66,24 @@ def _check_invariants(got, Xc, algo, K, what, recon_tol=2e-5):
 #    siblings of configs 2-5 whose sizes span several CTAs / tiles and have ragged tails.
 # --------------------------------------------------------------------------------------------
 SMALL_CASES = [
-    # (config index, M, N, K, path, ctas)     path: 0 auto, 1 streaming, 2 resident
+    # (config index, M, N, K, path, ctas)     path: 0 auto; two-sweep kernel 1 streaming, 2 resident;
+    #                                         single-sweep kernel 3 streaming, 4 resident
     (0, 256, 64, 8, 0, 0),          # BASELINE.json configs[0] in full, auto plan
     (0, 256, 64, 8, 1, 0),          # ... streaming plan
     (0, 256, 64, 8, 2, 7),          # ... resident, 7 CTAs (ragged row blocks)
+    (0, 256, 64, 8, 3, 0),          # ... single-sweep streaming, 148 CTAs (most own 2 rows, some none)
+    (0, 256, 64, 8, 4, 5),          # ... single-sweep resident, 5 CTAs
+    (1, 1000, 200, 6, 3, 0),        # row group = 32 threads, 2 float4 per thread, padded columns
+    (1, 1000, 200, 6, 4, 0),
+    (1, 1027, 131, 5, 3, 0),        # M % 4 != 0 and N % 4 != 0 (row-major working copy is padded)
+    (1, 1027, 131, 5, 4, 20),
+    (1, 3000, 700, 12, 3, 0),       # row group = 64 threads (2 warps: cross-warp reduction), NV = 3
+    (1, 3000, 700, 12, 4, 0),
+    (2, 2048, 512, 20, 3, 0),       # collinear columns, single-sweep streaming
+    (3, 8192, 256, 16, 3, 0),       # tall: many row batches per group
+    (3, 4096, 2048, 10, 3, 0),      # row group = 128 threads (config-4 column count)
+    (2, 1024, 4096, 6, 3, 0),       # row group = 256 threads (config-3 column count), M < N
+    (4, 1024, 64, 64, 4, 0),        # K = N full decomposition, single-sweep resident
     (1, 1000, 200, 6, 2, 0),        # M % 8 != 0, N % 8 != 0
     (1, 1000, 200, 6, 1, 0),
     (1, 1027, 131, 5, 1, 0),        # M % 4 != 0 -> scalar lane mapping
@@ -109,11 +123,12 @@ def test_paths_agree_and_are_deterministic(binding):
     each plan is bitwise reproducible run to run (fixed-order reductions)."""
     cfg = inputs.scaled(inputs.config(1), 1536, 384, K=6)
     pr = inputs.generate(cfg)
-    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2)]
-    for a, b in ((0, 1), (2, 3)):
+    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2, 3, 3, 4, 4)]
+    for a, b in ((0, 1), (2, 3), (4, 5), (6, 7)):
         for key in ("T", "P", "lam", "iters"):
             np.testing.assert_array_equal(runs[a][key], runs[b][key])
-    np.testing.assert_allclose(runs[0]["lam"], runs[2]["lam"], rtol=1e-5)
+    for r in runs[1:]:
+        np.testing.assert_allclose(runs[0]["lam"], r["lam"], rtol=1e-5)
 
 
 # --------------------------------------------------------------------------------------------
@@ -123,8 +138,11 @@ def test_eps_zero_runs_exactly_max_iter(binding):
     cfg = inputs.scaled(inputs.config(0), 256, 64, K=3)
     pr = inputs.generate(cfg)
     for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
-        got = binding.fit(pr.X, 3, 0.0, 7, algo)
-        assert got["iters"].tolist() == [7, 7, 7]
+        for path in (0, 1, 2, 3, 4):
+            got = binding.fit(pr.X, 3, 0.0, 7, algo, path=path)
+            assert got["iters"].tolist() == [7, 7, 7]
+        got = binding.fit(pr.X, 3, 0.0, 1, algo)               # a single pass per component
+        assert got["iters"].tolist() == [1, 1, 1]
 
 
 def test_eps_one_stops_at_second_pass(binding):

@@ -58,7 +58,27 @@ enum {
   PCA_OPT_PATH = 1,     /* 0 = auto; two-sweep kernel: 1 = HBM-streaming, 2 = SMEM-resident;
                            single-sweep kernel (R read once per inner pass): 3 = streaming, 4 = resident */
   PCA_OPT_CTAS = 2,     /* number of CTAs of the persistent kernel (0 = auto) */
-  PCA_OPT_CENTER_MODE = 3 /* 0 = column means (default), 1 = literal eq. (1) mean column */
+  PCA_OPT_CENTER_MODE = 3, /* 0 = column means (default), 1 = literal eq. (1) mean column */
+  PCA_OPT_TRACE = 4     /* single-sweep kernel only: capacity (records) of the device-side phase trace, 0 = off
+                           (default).  See pca_trace. */
+};
+
+/* Phase ids of the trace records (pca_trace).  One inner pass of the single-sweep kernel is
+ * PREADY -> SWEEP -> PUBLISHED -> X1 -> TEST -> QSLICE -> [APART -> X2 ->] PHAT -> X3 -> PREADY. */
+enum {
+  PCA_TR_COMPONENT = 1, /* component k starts (S1) */
+  PCA_TR_LOADS_DONE = 2,/* first sweep of the component done: pending deflation S9 + q = R^T t0 (S2), published */
+  PCA_TR_X1 = 3,        /* grid barrier 1 passed: all partial raw loads / |t~|^2 / B-partials visible */
+  PCA_TR_TEST = 4,      /* lambda' (S7) and the convergence test (S8) taken */
+  PCA_TR_QSLICE = 5,    /* slice owner: q slice combined and corrected to p~ = q - W B */
+  PCA_TR_APART = 6,     /* GS-PCA: partial A = P_(k)^T p~ published (S3, first half) */
+  PCA_TR_X2 = 7,        /* grid barrier 2 passed (GS-PCA, k > 0 only) */
+  PCA_TR_PHAT = 8,      /* slice owner: p^ = p~ - P A and its partial squared norm published (S3/S4) */
+  PCA_TR_X3 = 9,        /* grid barrier 3 passed */
+  PCA_TR_PREADY = 10,   /* unit loads p in shared memory (S4) */
+  PCA_TR_SWEEP = 11,    /* sweep over the CTA's rows done: t~ = R p (S5) and q = R^T t~ (S2 of the next pass) */
+  PCA_TR_PUBLISHED = 12,/* partial q, |t~|^2 and B-partials (S6) written to the exchange buffers */
+  PCA_TR_FINAL = 13     /* component finalised (T, P, lambda, iters, W column stored) */
 };
 
 /* Fields for pca_get_info. */
@@ -130,6 +150,14 @@ int pca_run(pca_ctx*, const float* X, float* T, float* P, float* lambda, int32_t
 /* Pointer to the residual R (dev, M x N, ld = M) inside the workspace; valid after a pca_run on
  * this context has completed ("return T, P, R"). */
 int pca_residual(const pca_ctx*, const float** R);
+
+/* Device-side phase trace of the last pca_run (tracing aid; PCA_OPT_TRACE > 0, single-sweep kernel).
+ *   records   dev pointer inside the workspace: records[0] = number of records written (<= capacity),
+ *             records[1 + i] = (phase id << 56) | (SM cycle counter of CTA 0 & (2^56 - 1)), in program order
+ *   capacity  the PCA_OPT_TRACE value
+ * Valid after the stream of pca_run has been synchronised; the caller copies it to the host.
+ * Errors: PCA_EINVAL, PCA_EUNSUPPORTED (trace off or two-sweep kernel), PCA_EWORKSPACE (no run yet). */
+int pca_trace(const pca_ctx*, const uint64_t** records, int64_t* capacity);
 
 /* Convenience entry with HOST buffers (used for end-to-end timing): copies X (host, M x N,
  * NOT centred) to the device, runs pca_center and pca_run on `stream`, copies T, P, lambda, iters

@@ -18,7 +18,7 @@ PCA_ALGO_GS = 1
 
 PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED = range(6)
 
-PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE = 1, 2, 3
+PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE = 1, 2, 3, 4
 PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT = 0, 1, 2, 3, 4
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
  PCA_INFO_LAUNCHES_PER_RUN, PCA_INFO_NUM_SMS, PCA_INFO_ROW_GROUP_THREADS) = range(1, 9)
@@ -26,7 +26,7 @@ PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, 
 EXPORTED_SYMBOLS = (
     "pca_create", "pca_set_option", "pca_get_info", "pca_workspace_bytes", "pca_set_workspace",
     "pca_center", "pca_run", "pca_residual", "pca_fit_host", "pca_destroy", "pca_strerror",
-    "pca_last_cuda_error",
+    "pca_last_cuda_error", "pca_trace",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -67,6 +67,7 @@ def load_library() -> ctypes.CDLL:
     lib.pca_strerror.argtypes = [i32]
     lib.pca_strerror.restype = ctypes.c_char_p
     lib.pca_last_cuda_error.argtypes = [vp]
+    lib.pca_trace.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i64)]
     _lib = lib
     return lib
 
@@ -174,6 +175,18 @@ class PcaContext:
         off = ptr.value - self._ws.data_ptr()
         nbytes = self.M * self.N * 4
         return self._ws[off:off + nbytes].view(torch.float32).view(self.N, self.M)
+
+    def pca_trace(self):
+        """Phase trace of the last pca_run as a (n, 2) int64 numpy array of (phase id, SM cycle counter)."""
+        import numpy as np
+        import torch
+        ptr, cap = ctypes.c_void_p(), ctypes.c_int64()
+        _check(self._lib.pca_trace(self._ctx, ctypes.byref(ptr), ctypes.byref(cap)), "pca_trace")
+        off = ptr.value - self._ws.data_ptr()
+        rec = self._ws[off:off + 8 * (cap.value + 1)].view(torch.int64).cpu().numpy()
+        n = int(rec[0])
+        body = rec[1:1 + n]
+        return np.stack([(body >> 56) & 0xff, body & ((1 << 56) - 1)], axis=1)
 
     def pca_fit_host(self, X_host, T_host, P_host, lam_host, iters_host, stream=None) -> None:
         """Host (CPU, ideally pinned) torch tensors: X (N,M) NOT centred in; T (K,M), P (K,N), lam, iters out."""

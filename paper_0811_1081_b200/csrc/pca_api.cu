@@ -59,7 +59,7 @@ struct pca_ctx {
   // device
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
-  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0;
+  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel)
@@ -68,7 +68,7 @@ struct pca_ctx {
   const FusedVariant* fvariant = nullptr;
   FusedParams fprm{};
   size_t ws_off_rrm = 0, ws_off_qpart2 = 0, ws_off_bpart2 = 0, ws_off_spart2 = 0, ws_off_apart2 = 0, ws_off_pvec2 = 0,
-         ws_off_npart = 0, ws_off_w = 0;
+         ws_off_npart = 0, ws_off_w = 0, ws_off_trace = 0;
   size_t smem_bytes = 0;
   size_t ws_bytes = 0;
   size_t ws_off_ppart = 0, ws_off_apart = 0, ws_off_bpart = 0, ws_off_pvec = 0, ws_off_qpart = 0, ws_off_spart = 0,
@@ -231,6 +231,8 @@ int make_fused_plan(pca_ctx* c, int want) {
   c->ws_off_pvec2 = take((size_t)ldr * 4);
   c->ws_off_npart = take((size_t)p.Gs * 8);
   c->ws_off_w = take((size_t)ldr * p.Kpad * 4);
+  c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1) * 8 : 0);
+  p.trace_cap = c->opt_trace;
   c->ws_off_bar = take(256);
   c->ws_bytes = off;
   c->fprm = p;
@@ -369,6 +371,10 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
       if (value < 0 || value > 1) return PCA_EINVAL;
       c->opt_center_mode = (int)value;
       return PCA_OK;
+    case PCA_OPT_TRACE:
+      if (value < 0 || value > (1 << 24)) return PCA_EINVAL;
+      c->opt_trace = (int)value;
+      break;
     default:
       return PCA_EINVAL;
   }
@@ -436,7 +442,9 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     p.Npart = reinterpret_cast<double*>(ws + c->ws_off_npart);
     p.W = reinterpret_cast<float*>(ws + c->ws_off_w);
     p.bar = reinterpret_cast<unsigned long long*>(ws + c->ws_off_bar);
+    p.trace = reinterpret_cast<unsigned long long*>(ws + c->ws_off_trace);
     PCA_CUDA(c, cudaMemsetAsync(p.bar, 0, 256, st));
+    if (p.trace_cap > 0) PCA_CUDA(c, cudaMemsetAsync(p.trace, 0, 8, st));
     const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
     pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X
     PCA_CUDA(c, cudaGetLastError());
@@ -474,6 +482,15 @@ int pca_residual(const pca_ctx* c, const float** R) {
   if (!c || !R) return PCA_EINVAL;
   if (!c->ws || !c->ran) return PCA_EWORKSPACE;
   *R = reinterpret_cast<const float*>(c->ws);
+  return PCA_OK;
+}
+
+int pca_trace(const pca_ctx* c, const uint64_t** records, int64_t* capacity) {
+  if (!c || !records || !capacity) return PCA_EINVAL;
+  if (!c->planned || c->path < 3 || c->opt_trace <= 0) return PCA_EUNSUPPORTED;
+  if (!c->ws || !c->ran) return PCA_EWORKSPACE;
+  *records = reinterpret_cast<const uint64_t*>(static_cast<const unsigned char*>(c->ws) + c->ws_off_trace);
+  *capacity = c->opt_trace;
   return PCA_OK;
 }
 

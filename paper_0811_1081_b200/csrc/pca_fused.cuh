@@ -63,11 +63,23 @@ struct FusedParams {
   double* Npart;         // [Gs]         partial |p^|^2
   float* W;              // [ldr][Kpad]  W = R^T V
   unsigned long long* bar;
+  unsigned long long* trace;  // optional phase trace (PCA_OPT_TRACE): [0] = records written, then records
+  int trace_cap;              // capacity in records (0 = off)
   // shared-memory carve-up (byte offsets)
   int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_slab;
 };
 
 constexpr int kRB = 4;   // rows per batch
+
+// Phase trace (include/pca.h, PCA_OPT_TRACE): thread 0 of CTA 0 appends (phase << 56) | clock64().
+enum { TR_COMPONENT = 1, TR_LOADS_DONE = 2, TR_X1 = 3, TR_TEST = 4, TR_QSLICE = 5, TR_APART = 6, TR_X2 = 7,
+       TR_PHAT = 8, TR_X3 = 9, TR_PREADY = 10, TR_SWEEP = 11, TR_PUBLISHED = 12, TR_FINAL = 13 };
+__device__ __forceinline__ void trace_mark(const FusedParams& prm, int& tn, int phase) {
+  if (prm.trace_cap > 0 && blockIdx.x == 0 && threadIdx.x == 0 && tn < prm.trace_cap) {
+    prm.trace[1 + tn] = ((unsigned long long)phase << 56) | ((unsigned long long)clock64() & 0x00ffffffffffffffULL);
+    ++tn;
+  }
+}
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -309,6 +321,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
   const int ns = max(0, min(prm.Ns, N - n0));
   unsigned long long bar_target = 0;
   unsigned sweep_no = 0;                                   // parity selects the exchange buffers
+  int tn = 0;                                              // trace records written (thread 0 of CTA 0)
 
   float* Rb = prm.Rrm + (size_t)m0 * ldr;
   float* Tb = prm.T + m0;
@@ -319,6 +332,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
 
   for (int k = 0; k < K; ++k) {
     const bool gsk = gs && k > 0;
+    trace_mark(prm, tn, TR_COMPONENT);
     // ---- S1: t0 <- column k of the deflated residual (reading C6) ----
     for (int i = tid; i < mb; i += kThreads) {
       float r;
@@ -343,6 +357,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       s = block_sum(s, scr);
       if (tid == 0) prm.Spart[(size_t)buf * G + b] = s;
     }
+    trace_mark(prm, tn, TR_LOADS_DONE);
 
     double lam = 0.0, lam_new = 0.0;
     int it = 0;
@@ -352,6 +367,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       const unsigned buf = sweep_no & 1u;
       const float* Qp = prm.Qpart + (size_t)buf * G * ldr;
       grid_barrier(prm.bar, bar_target, G);                                   // ---- X1 ----
+      trace_mark(prm, tn, TR_X1);
       const double s = sum_parts(prm.Spart + (size_t)buf * G, G, scr);
       bool done = false;
       if (first) {
@@ -371,6 +387,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         done = (fabs(lam - lam_new) < prm.eps * lam_new) || (it >= prm.max_iter);
         if (!done) lam = lam_new;
       }
+      trace_mark(prm, tn, TR_TEST);
       // ---- owners: q_S = sum of the G partials, fixed order, fp64 ----
       const bool need_q = !done || (gs && k + 1 < K);                         // finalize needs q only for W_k
       if (ns > 0 && need_q) {
@@ -406,6 +423,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         }
       }
       if (done) break;
+      trace_mark(prm, tn, TR_QSLICE);
 
       if (gsk) {
         // ---- S3: A-partials a_S[j] = sum_{n in S} P[n,j] p~[n] ----
@@ -417,7 +435,9 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
             prm.Apart[(size_t)b * Kpad + j] = (float)a;
           }
         }
+        trace_mark(prm, tn, TR_APART);
         grid_barrier(prm.bar, bar_target, G);                                 // ---- X2 ----
+        trace_mark(prm, tn, TR_X2);
         if (ns > 0) {
           reduce_fparts(A_s, prm.Apart, k, prm.Gs, Kpad, scr);
           // p^ = p~ - P_(k) A
@@ -448,13 +468,16 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         q2 = block_sum(q2, scr);
         if (tid == 0) prm.Npart[b] = q2;
       }
+      trace_mark(prm, tn, TR_PHAT);
       grid_barrier(prm.bar, bar_target, G);                                   // ---- X3 ----
+      trace_mark(prm, tn, TR_X3);
       const double pn2 = sum_parts(prm.Npart, prm.Gs, scr);
       if (!(pn2 > 0.0)) { degenerate = true; break; }                         // reading C7
       const float inv_pn = (float)(1.0 / sqrt(pn2));                          // p = p^/|p^|
       for (int n = tid; n < ldr; n += kThreads) p_s[n] = (n < N) ? ld_cg(prm.pvec + n) * inv_pn : 0.f;
       __syncthreads();
       first = false;
+      trace_mark(prm, tn, TR_PREADY);
       // ---- FUSED sweep: t~ = R p (S5), q = R^T t~, s = |t~|^2 ----
       ++sweep_no;
       ++it;
@@ -463,6 +486,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         const bool rev = (sweep_no & 1u) != 0;
         if constexpr (RESIDENT) sweep_fused<NV, SRC_SLAB>(prm, Rb, slab, mb, p_s, ttil_s, qs, red_s, sgrp, false);
         else                    sweep_fused<NV, SRC_GLOBAL>(prm, Rb, slab, mb, p_s, ttil_s, qs, red_s, sgrp, rev);
+        trace_mark(prm, tn, TR_SWEEP);
         publish_q(prm, qs, prm.Qpart + ((size_t)nbuf * G + b) * ldr);
         if (tid == 0) {
           double a = 0.0;
@@ -479,6 +503,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
             if (lane == 0) bp[j] = (float)sj;
           }
         }
+        trace_mark(prm, tn, TR_PUBLISHED);
       }
     }
 
@@ -518,7 +543,9 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
     }
     ++sweep_no;                                                               // next LOADS sweep takes the other buffers
     __syncthreads();
+    trace_mark(prm, tn, TR_FINAL);
   }
+  if (prm.trace_cap > 0 && b == 0 && tid == 0) prm.trace[0] = (unsigned long long)tn;
 
   // resident: hand the slab back (the last deflation is applied by pca_transpose_out_kernel)
   if constexpr (RESIDENT) sweep_loads<NV, SRC_SLAB, DST_GLOBAL, false, false>(prm, Rb, slab, mb, ttil_s, d_s, pdef_s, qs);

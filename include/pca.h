@@ -90,7 +90,9 @@ enum {
   PCA_INFO_ROWS_PER_CTA = 5,
   PCA_INFO_LAUNCHES_PER_RUN = 6, /* kernel launches one pca_run enqueues */
   PCA_INFO_NUM_SMS = 7,
-  PCA_INFO_ROW_GROUP_THREADS = 8 /* single-sweep kernel: threads that share one row of R (0 otherwise) */
+  PCA_INFO_ROW_GROUP_THREADS = 8, /* single-sweep kernel: threads that share one row of R (0 otherwise) */
+  PCA_INFO_RUN_STATUS = 9   /* SYNCHRONISES the device and reads the status word of the last pca_run: 0 = ok,
+                               1 = a cross-CTA exchange wait gave up (results invalid; never in a correct run) */
 };
 
 /* Create a context for one problem shape.

@@ -67,8 +67,8 @@ struct pca_ctx {
   SolveParams prm{};
   const FusedVariant* fvariant = nullptr;
   FusedParams fprm{};
-  size_t ws_off_rrm = 0, ws_off_qpart2 = 0, ws_off_bpart2 = 0, ws_off_spart2 = 0, ws_off_apart2 = 0, ws_off_pvec2 = 0,
-         ws_off_npart = 0, ws_off_w = 0, ws_off_trace = 0;
+  size_t ws_off_rrm = 0, ws_off_xchg = 0, ws_xchg_bytes = 0, ws_off_qx = 0, ws_off_sbx = 0, ws_off_ax = 0, ws_off_px = 0,
+         ws_off_nx = 0, ws_off_pown = 0, ws_off_wown = 0, ws_off_status = 0, ws_off_cnt = 0, ws_off_trace = 0;
   size_t smem_bytes = 0;
   size_t ws_bytes = 0;
   size_t ws_off_ppart = 0, ws_off_apart = 0, ws_off_bpart = 0, ws_off_pvec = 0, ws_off_qpart = 0, ws_off_spart = 0,
@@ -165,18 +165,25 @@ int make_fused_plan(pca_ctx* c, int want) {
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 16); return (int)o; };
     const size_t mbp = (size_t)round_up(p->Mb, 4);
-    p->off_p = take((size_t)ldr * 4);
+    const size_t npx = (size_t)p->Gs * p->Ns;
+    p->off_p = take((npx > (size_t)ldr ? npx : (size_t)ldr) * 4);
     p->off_pdef = take((size_t)ldr * 4);
     p->off_ttil = take(mbp * 4);
     p->off_d = take(mbp * 4);
     p->off_qs = take((size_t)pca::kThreads * 4 * NV * 4);
     p->off_red = take((size_t)2 * pca::kWarps * pca::kRB * 4);
     p->off_sgrp = take((size_t)(pca::kThreads / GT) * 8);
-    p->off_B = take((size_t)p->Kpad * 8);
+    p->off_B = take((size_t)(2 + p->Kpad) * 8);
     p->off_A = take((size_t)p->Kpad * 8);
     p->off_scr = take((size_t)pca::kThreads * 8);
     p->off_praw = take((size_t)p->Ns * 8);
     p->off_lam = take((size_t)p->Kpad * 4);
+    // owner-private panels P[slice, :], W[slice, :]: shared memory unless that crowds out the rest
+    const size_t panel = (size_t)p->Ns * p->Kpad * 4;
+    const size_t slab_bytes = resident ? (size_t)p->Mb * (size_t)ldr * 4 : 0;
+    p->cache_pw = (off + 2 * panel + slab_bytes <= (size_t)c->smem_optin && 2 * panel <= (size_t)64 * 1024) ? 1 : 0;
+    p->off_pc = take(p->cache_pw ? panel : 0);
+    p->off_wc = take(p->cache_pw ? panel : 0);
     p->off_slab = take(resident ? (size_t)p->Mb * (size_t)ldr * 4 : 0);
     return off;
   };
@@ -224,16 +231,20 @@ int make_fused_plan(pca_ctx* c, int want) {
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
   take((size_t)M * (size_t)N * 4);                                   // residual of eq. (4), column-major (ABI layout)
   c->ws_off_rrm = take((size_t)M * (size_t)ldr * 4);                 // working residual, row-major
-  c->ws_off_qpart2 = take((size_t)2 * p.G * ldr * 4);
-  c->ws_off_bpart2 = take((size_t)2 * p.G * p.Kpad * 4);
-  c->ws_off_spart2 = take((size_t)2 * p.G * 8);
-  c->ws_off_apart2 = take((size_t)p.Gs * p.Kpad * 4);
-  c->ws_off_pvec2 = take((size_t)ldr * 4);
-  c->ws_off_npart = take((size_t)p.Gs * 8);
-  c->ws_off_w = take((size_t)ldr * p.Kpad * 4);
+  // LL exchange buffers + status word: one contiguous region, zeroed before every launch
+  c->ws_off_xchg = off;
+  c->ws_off_qx = take((size_t)2 * p.Gs * p.G * p.Ns * 8);
+  c->ws_off_sbx = take((size_t)2 * p.G * (2 + p.Kpad) * 8);
+  c->ws_off_ax = take((size_t)2 * p.Gs * p.Kpad * 8);
+  c->ws_off_px = take((size_t)2 * p.Gs * p.Ns * 8);
+  c->ws_off_nx = take((size_t)2 * p.Gs * 2 * 8);
+  c->ws_off_pown = take(p.cache_pw ? 0 : (size_t)p.Gs * p.Ns * p.Kpad * 4);
+  c->ws_off_wown = take(p.cache_pw ? 0 : (size_t)p.Gs * p.Ns * p.Kpad * 4);
+  c->ws_off_status = take(256);
+  c->ws_off_cnt = take(1024);
+  c->ws_xchg_bytes = off - c->ws_off_xchg;
   c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1) * 8 : 0);
   p.trace_cap = c->opt_trace;
-  c->ws_off_bar = take(256);
   c->ws_bytes = off;
   c->fprm = p;
   c->fvariant = var;
@@ -392,6 +403,16 @@ int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
     case PCA_INFO_LAUNCHES_PER_RUN: *value = c->path >= 3 ? 3 : 1; break;
     case PCA_INFO_ROW_GROUP_THREADS: *value = c->path >= 3 ? c->fprm.GT : 0; break;
     case PCA_INFO_NUM_SMS: *value = c->num_sms; break;
+    case PCA_INFO_RUN_STATUS: {
+      *value = 0;
+      if (c->path >= 3 && c->ws && c->ran) {
+        unsigned st = 0;
+        if (cudaMemcpy(&st, static_cast<const unsigned char*>(c->ws) + c->ws_off_status, sizeof(st),
+                       cudaMemcpyDeviceToHost) != cudaSuccess) return PCA_ECUDA;
+        *value = (int64_t)st;
+      }
+      break;
+    }
     default: return PCA_EINVAL;
   }
   return PCA_OK;
@@ -434,16 +455,18 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     FusedParams p = c->fprm;
     p.Rrm = reinterpret_cast<float*>(ws + c->ws_off_rrm);
     p.T = T; p.P = P; p.lambda = lambda; p.iters = iters;
-    p.Qpart = reinterpret_cast<float*>(ws + c->ws_off_qpart2);
-    p.Bpart = reinterpret_cast<float*>(ws + c->ws_off_bpart2);
-    p.Spart = reinterpret_cast<double*>(ws + c->ws_off_spart2);
-    p.Apart = reinterpret_cast<float*>(ws + c->ws_off_apart2);
-    p.pvec = reinterpret_cast<float*>(ws + c->ws_off_pvec2);
-    p.Npart = reinterpret_cast<double*>(ws + c->ws_off_npart);
-    p.W = reinterpret_cast<float*>(ws + c->ws_off_w);
-    p.bar = reinterpret_cast<unsigned long long*>(ws + c->ws_off_bar);
+    typedef unsigned long long u64;
+    p.Qx = reinterpret_cast<u64*>(ws + c->ws_off_qx);
+    p.SBx = reinterpret_cast<u64*>(ws + c->ws_off_sbx);
+    p.Ax = reinterpret_cast<u64*>(ws + c->ws_off_ax);
+    p.Px = reinterpret_cast<u64*>(ws + c->ws_off_px);
+    p.Nx = reinterpret_cast<u64*>(ws + c->ws_off_nx);
+    p.Pown = reinterpret_cast<float*>(ws + c->ws_off_pown);
+    p.Wown = reinterpret_cast<float*>(ws + c->ws_off_wown);
+    p.status = reinterpret_cast<unsigned*>(ws + c->ws_off_status);
+    p.cnt = reinterpret_cast<unsigned*>(ws + c->ws_off_cnt);
     p.trace = reinterpret_cast<unsigned long long*>(ws + c->ws_off_trace);
-    PCA_CUDA(c, cudaMemsetAsync(p.bar, 0, 256, st));
+    PCA_CUDA(c, cudaMemsetAsync(ws + c->ws_off_xchg, 0, c->ws_xchg_bytes, st));   // sequence numbers start at 0
     if (p.trace_cap > 0) PCA_CUDA(c, cudaMemsetAsync(p.trace, 0, 8, st));
     const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
     pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X

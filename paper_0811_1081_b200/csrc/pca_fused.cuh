@@ -26,12 +26,15 @@
 // Per component k:
 //   t0 <- column k of the deflated residual                                   (S1)
 //   LOADS sweep : R <- R - d p_prev^T (pending deflation S9, stored), q = R^T t0, s = |t0|^2
-//   loop: [X1] s, B known everywhere -> lambda', test (S7, S8) -> owners: p~ = q - W B, A-partials
-//         [X2] A -> p^ = p~ - P A, |p^|^2 partials (S3)     (GS-PCA and k > 0 only)
-//         [X3] p = p^/|p^| everywhere (S4) -> FUSED sweep: t~ = R p (S5), q = R^T t~ (S2 of the
-//              next pass), s = |t~|^2, B-partials = V^T t~ (S6)
+//   loop: [hop 1] s, B everywhere -> lambda', test (S7, S8);  slice owners: q slice -> p~ = q - W B, A-partials
+//         [hop 2] owners: A -> p^ = p~ - P A, |p^|^2 partials (S3)     (GS-PCA and k > 0 only)
+//         [hop 3] p = p^/|p^| everywhere (S4) -> FUSED sweep: t~ = R p (S5), q = R^T t~ (S2 of the
+//                 next pass), s = |t~|^2, B-partials = V^T t~ (S6)
 //   finalize: t = t~ - V B, v = t/lambda', store T, P, lambda, iters, W_k; d <- t
-// [X1..X3] are grid barriers; every CTA takes the same decisions from the same reduced values.
+// The hops are NOT grid barriers: data travels between CTAs in self-validating 8-byte words
+// {payload, sequence number} (see "LL exchange" below), so a hop costs one store and one polling
+// load through L2 (measured: a counter barrier + reduction phase cost 2-6 us, pca_trace).  Every
+// CTA takes the same decisions from the same reduced values (fixed summation order, fp64).
 // =====================================================================================
 #pragma once
 #include "pca_device.cuh"
@@ -55,18 +58,22 @@ struct FusedParams {
   int GT;                // threads that share one row (power of two, 32..512)
   int Ns, Gs;            // columns per slice owner, number of owners
   int Kpad;
-  float* Qpart;          // [2][G][ldr]  partial raw loads (double-buffered by sweep parity)
-  float* Bpart;          // [2][G][Kpad] partial B
-  double* Spart;         // [2][G]       partial |t~|^2
-  float* Apart;          // [Gs][Kpad]   partial A
-  float* pvec;           // [ldr]        p^ (orthogonalised, not normalised)
-  double* Npart;         // [Gs]         partial |p^|^2
-  float* W;              // [ldr][Kpad]  W = R^T V
-  unsigned long long* bar;
+  // LL exchange buffers: 8-byte words {payload, seq}, double-buffered by sweep parity (see "LL exchange" below)
+  unsigned long long* Qx;   // [2][Gs][G][Ns]   partial raw loads, grouped by slice owner
+  unsigned long long* SBx;  // [2][G][2 + Kpad] words 0-1: partial |t~|^2 (fp64 bits); word 2+j: partial B[j]
+  unsigned long long* Ax;   // [2][Gs][Kpad]    partial A
+  unsigned long long* Px;   // [2][Gs*Ns]       p^ (orthogonalised, not normalised)
+  unsigned long long* Nx;   // [2][Gs][2]       partial |p^|^2 (fp64 bits)
+  float* Pown;              // [Gs][Ns][Kpad]   owner-private panels P[slice, :], W[slice, :] (W = R^T V) when
+  float* Wown;              //                  they do not fit in shared memory (cache_pw == 0)
+  int cache_pw;
+  unsigned* status;         // [0] != 0: an exchange wait gave up (kSpinLimit)
+  unsigned* cnt;            // arrival-counter hints of the three hops, 64 words apart (relaxed; see hop_arrive/hop_wait)
   unsigned long long* trace;  // optional phase trace (PCA_OPT_TRACE): [0] = records written, then records
   int trace_cap;              // capacity in records (0 = off)
   // shared-memory carve-up (byte offsets)
-  int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_slab;
+  int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_pc, off_wc,
+      off_slab;
 };
 
 constexpr int kRB = 4;   // rows per batch
@@ -74,9 +81,15 @@ constexpr int kRB = 4;   // rows per batch
 // Phase trace (include/pca.h, PCA_OPT_TRACE): thread 0 of CTA 0 appends (phase << 56) | clock64().
 enum { TR_COMPONENT = 1, TR_LOADS_DONE = 2, TR_X1 = 3, TR_TEST = 4, TR_QSLICE = 5, TR_APART = 6, TR_X2 = 7,
        TR_PHAT = 8, TR_X3 = 9, TR_PREADY = 10, TR_SWEEP = 11, TR_PUBLISHED = 12, TR_FINAL = 13 };
+// BAR.SYNC does not block at issue: a stamp right after __syncthreads() would be the barrier's ISSUE time.  The
+// shared-memory read below depends on the barrier's release, and the clock read depends on its value.
 __device__ __forceinline__ void trace_mark(const FusedParams& prm, int& tn, int phase) {
   if (prm.trace_cap > 0 && blockIdx.x == 0 && threadIdx.x == 0 && tn < prm.trace_cap) {
-    prm.trace[1 + tn] = ((unsigned long long)phase << 56) | ((unsigned long long)clock64() & 0x00ffffffffffffffULL);
+    extern __shared__ __align__(16) unsigned char trace_smem_[];
+    const unsigned dep = *reinterpret_cast<volatile unsigned*>(trace_smem_);
+    unsigned long long c;
+    asm volatile("{ .reg .u32 t; and.b32 t, %1, 0; mov.u64 %0, %%clock64; }" : "=l"(c) : "r"(dep) : "memory");
+    prm.trace[1 + tn] = ((unsigned long long)phase << 56) | (c & 0x00ffffffffffffffULL);
     ++tn;
   }
 }
@@ -252,59 +265,156 @@ __device__ __forceinline__ void sweep_fused(const FusedParams& prm, const float*
   __syncthreads();
 }
 
-// Combine the NG group partials and publish this CTA's partial raw loads (fixed order).
-__device__ __forceinline__ void publish_q(const FusedParams& prm, const float* qs, float* qpart_row) {
-  const int NG = kThreads / prm.GT, ldr = prm.ldr;
-  for (int c = threadIdx.x * 4; c < ldr; c += kThreads * 4) {
-    float4 a = *reinterpret_cast<const float4*>(qs + c);
-    for (int g = 1; g < NG; ++g) {
-      const float4 b = *reinterpret_cast<const float4*>(qs + (size_t)g * ldr + c);
-      a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
-    }
-    *reinterpret_cast<float4*>(qpart_row + c) = a;
+// ------------------------------------------------------------------------------------ LL exchange
+// Cross-CTA exchange without grid barriers.  Every exchanged 32-bit payload travels in an 8-byte
+// word {payload, seq}: the word is written with ONE 64-bit store (single-copy atomic), so a reader
+// that sees the expected sequence number also sees the payload -- no fence, no flag, no barrier;
+// a hop costs one store and one (polling) load through L2.  seq = number of the sweep that
+// produced the data (1, 2, ...; the buffers are zeroed before the launch).  All buffers are
+// double-buffered by the parity of seq: a CTA can only be one sweep ahead of the slowest reader
+// (it needs the loads p of sweep s+1, which every slice owner publishes only after it has read
+// the partials of sweep s from ALL CTAs), so a word of sweep s is never overwritten (by sweep
+// s+2) while somebody still waits for it.
+// Pairs of words are moved with 16-byte vector accesses (two independent 8-byte atomic halves).
+typedef unsigned long long u64;
+constexpr unsigned kSpinLimit = 1u << 22;   // polls before a wait gives up and raises status[0] (never in a correct run)
+
+__device__ __forceinline__ u64 ll_word(unsigned payload, unsigned seq) { return ((u64)seq << 32) | (u64)payload; }
+__device__ __forceinline__ u64 ll_wordf(float v, unsigned seq) { return ll_word(__float_as_uint(v), seq); }
+__device__ __forceinline__ float ll_f(u64 w) { return __uint_as_float((unsigned)w); }
+__device__ __forceinline__ void ll_st2(u64* p, u64 a, u64 b) {
+  asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ void ll_ld2(const u64* p, u64& a, u64& b) {
+  asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void ll_st2d(u64* p, double v, unsigned seq) {      // one fp64 value in two words (lossless)
+  const u64 bits = (u64)__double_as_longlong(v);
+  ll_st2(p, ll_word((unsigned)bits, seq), ll_word((unsigned)(bits >> 32), seq));
+}
+__device__ __forceinline__ double ll_d(u64 a, u64 b) {
+  return __longlong_as_double((long long)((b << 32) | (a & 0xffffffffULL)));
+}
+__device__ __forceinline__ void ll_wait2(const u64* p, unsigned seq, u64& a, u64& b, unsigned* status) {
+  unsigned spins = 0;
+  while ((unsigned)(a >> 32) != seq || (unsigned)(b >> 32) != seq) {
+    ll_ld2(p, a, b);
+    if (++spins > kSpinLimit) { *status = 1u; break; }
   }
 }
 
-// out_s[j] = sum_{b < nparts} part[b*stride + j] (float partials, fp64 sums, fixed order), j < count.
-__device__ __forceinline__ void reduce_fparts(double* out_s, const float* part, int count, int nparts, int stride,
-                                              double* scr) {
-  for (int j0 = 0; j0 < count; j0 += kThreads) {
-    const int cnt = min(count - j0, kThreads);
-    const int cp = (cnt + 31) & ~31;
-    int nsub = kThreads / cp;
-    if (nsub > nparts) nsub = nparts;
-    const int sub = threadIdx.x / cp, j = threadIdx.x - sub * cp;
-    double v = 0.0;
-    if (sub < nsub && j < cnt) {
-      const float* src = part + j0 + j;
-#pragma unroll 4
-      for (int b = sub; b < nparts; b += nsub) v += (double)ld_cg(src + (size_t)b * stride);
+// Arrival hints.  Thousands of threads polling the same words delay the very stores they wait for (measured: 3000-6000
+// cycles per hop).  So a producer CTA, after its LL stores, bumps a RELAXED counter, and only thread 0 of a consumer
+// CTA polls that counter; the other threads sleep at the block barrier.  The counter orders nothing (no fence): it only
+// says "the data is probably there"; the sequence numbers in the data words remain the correctness mechanism.
+__device__ __forceinline__ void hop_arrive(unsigned* ctr) {         // call by ONE thread after a block/warp barrier
+  asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
+}
+__device__ __forceinline__ void hop_wait(const unsigned* ctr, unsigned expected, unsigned* status) {
+  if (threadIdx.x == 0) {
+    unsigned v, spins = 0;
+    for (;;) {
+      asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+      if ((int)(v - expected) >= 0) break;
+      if (++spins > kSpinLimit) { *status = 1u; break; }
     }
-    __syncthreads();
-    if (sub < nsub) scr[sub * cp + j] = v;
-    __syncthreads();
-    if (threadIdx.x < cnt) {
-      double s = 0.0;
-      for (int q = 0; q < nsub; ++q) s += scr[q * cp + threadIdx.x];
-      out_s[j0 + threadIdx.x] = s;
+  }
+  __syncthreads();
+}
+
+// One reduction job: out[j] = sum over parts b < nparts of word (base + b*stride)[j], j < 2*units, fp64, fixed order
+// (lane l takes parts l, l+32, ... in order, then a shuffle tree).  If f64_unit0, words 0-1 hold one fp64 value.
+struct LLJob {
+  const u64* base;
+  double* out;
+  int units, nparts, stride;
+  bool f64_unit0;
+};
+constexpr int kLLParts = 5;                 // parts per lane held in flight (covers 160 CTAs in one round)
+
+__device__ __forceinline__ void ll_reduce_unit(const LLJob& jb, int u, unsigned seq, unsigned* status) {
+  const int lane = threadIdx.x & 31;
+  double a0 = 0.0, a1 = 0.0;
+  for (int b0 = lane; b0 < jb.nparts; b0 += 32 * kLLParts) {
+    u64 x[kLLParts], y[kLLParts];
+#pragma unroll
+    for (int i = 0; i < kLLParts; ++i) {
+      const int bq = b0 + 32 * i;
+      x[i] = 0; y[i] = 0;
+      if (bq < jb.nparts) ll_ld2(jb.base + (size_t)bq * jb.stride + 2 * u, x[i], y[i]);
     }
-    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kLLParts; ++i) {
+      const int bq = b0 + 32 * i;
+      if (bq < jb.nparts) {
+        ll_wait2(jb.base + (size_t)bq * jb.stride + 2 * u, seq, x[i], y[i], status);
+        if (jb.f64_unit0 && u == 0) a0 += ll_d(x[i], y[i]);
+        else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
+      }
+    }
+  }
+  a0 = warp_sum(a0);
+  a1 = warp_sum(a1);
+  if (lane == 0) { jb.out[2 * u] = a0; jb.out[2 * u + 1] = a1; }
+}
+
+// Two jobs share the 16 warps of the CTA (one warp per 2-word unit).  No barrier inside.
+__device__ __forceinline__ void ll_reduce2(const LLJob& ja, const LLJob& jb, unsigned seq, unsigned* status) {
+  const int w = threadIdx.x >> 5;
+  const int total = ja.units + jb.units;
+  for (int uu = w; uu < total; uu += kWarps) {
+    if (uu < ja.units) ll_reduce_unit(ja, uu, seq, status);
+    else ll_reduce_unit(jb, uu - ja.units, seq, status);
+  }
+}
+
+// Combine the NG group partials of the sweep (fixed order) and publish this CTA's partial raw loads:
+// column c of slice owner o = c / Ns goes to Qpar[(o*G + b)*Ns + c % Ns]   (S2)
+__device__ __forceinline__ void publish_q_ll(const FusedParams& prm, const float* qs, u64* Qpar, int b, unsigned seq) {
+  const int NG = kThreads / prm.GT, ldr = prm.ldr, Ns = prm.Ns;
+  const int ncol = prm.Gs * Ns;
+  for (int c = threadIdx.x * 2; c < ncol; c += kThreads * 2) {
+    float2 a = make_float2(0.f, 0.f);
+    if (c < ldr) {
+      a = *reinterpret_cast<const float2*>(qs + c);
+      for (int g = 1; g < NG; ++g) {
+        const float2 v = *reinterpret_cast<const float2*>(qs + (size_t)g * ldr + c);
+        a.x += v.x; a.y += v.y;
+      }
+    }
+    const int o = c / Ns, i = c - o * Ns;
+    ll_st2(Qpar + ((size_t)o * prm.G + b) * Ns + i, ll_wordf(a.x, seq), ll_wordf(a.y, seq));
+  }
+}
+
+// praw[i] -= sum_{j<k} C[i*Kpad + j] * coef[j] for the ns columns of this owner (one warp per column).
+__device__ __forceinline__ void slice_correct(double* praw_s, const float* C, const double* coef_s, int ns, int k, int Kpad,
+                                              int w0 = 0) {                  // warps w0..kWarps-1 take part
+  const int lane = threadIdx.x & 31, w = (threadIdx.x >> 5) - w0;
+  for (int i = w; i < ns; i += kWarps - w0) {
+    const float* ci = C + (size_t)i * Kpad;
+    double c = 0.0;
+    for (int j = lane; j < k; j += 32) c += (double)ci[j] * coef_s[j];
+    c = warp_sum(c);
+    if (lane == 0) praw_s[i] -= c;
   }
 }
 
 template <int NV, bool RESIDENT>
 __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParams prm) {
   extern __shared__ __align__(16) unsigned char smem[];
-  float* p_s = reinterpret_cast<float*>(smem + prm.off_p);        // ldr: current unit loads p
+  float* p_s = reinterpret_cast<float*>(smem + prm.off_p);        // npx: current unit loads p
   float* pdef_s = reinterpret_cast<float*>(smem + prm.off_pdef);  // ldr: loads of the previous component
   float* ttil_s = reinterpret_cast<float*>(smem + prm.off_ttil);  // Mb : t0 / t~ rows of this CTA
   float* d_s = reinterpret_cast<float*>(smem + prm.off_d);        // Mb : pending deflation vector rows
   float* qs = reinterpret_cast<float*>(smem + prm.off_qs);        // NG x ldr group partials
   float* red_s = reinterpret_cast<float*>(smem + prm.off_red);    // 2 x kWarps x kRB
   double* sgrp = reinterpret_cast<double*>(smem + prm.off_sgrp);  // NG
-  double* B_s = reinterpret_cast<double*>(smem + prm.off_B);      // Kpad
+  double* sb_s = reinterpret_cast<double*>(smem + prm.off_B);     // 2 + Kpad: |t~|^2, -, B
+  double* B_s = sb_s + 2;
   double* A_s = reinterpret_cast<double*>(smem + prm.off_A);      // Kpad
   double* scr = reinterpret_cast<double*>(smem + prm.off_scr);    // kThreads
+  double* ctl_s = scr + kThreads - 4;                             // lambda', decision, 1/|p^| of the current pass
   double* praw_s = reinterpret_cast<double*>(smem + prm.off_praw);// Ns: p~ / p^ slice of this owner
   float* lam_s = reinterpret_cast<float*>(smem + prm.off_lam);    // Kpad
   float* slab = reinterpret_cast<float*>(smem + prm.off_slab);    // resident: Mb x ldr
@@ -312,22 +422,38 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
   const long long M = prm.M;
-  const int N = prm.N, K = prm.K, G = prm.G, ldr = prm.ldr, Kpad = prm.Kpad;
+  const int N = prm.N, K = prm.K, G = prm.G, ldr = prm.ldr, Kpad = prm.Kpad, Ns = prm.Ns, Gs = prm.Gs;
   const int NG = kThreads / prm.GT;
+  const int npx = Gs * Ns;                                 // exchanged length of p (>= N)
+  const int SBw = 2 + Kpad;
   const bool gs = prm.algo == 1;
   const long long m0 = (long long)b * prm.Mb;
   const int mb = (int)max(0LL, min((long long)prm.Mb, M - m0));
-  const int n0 = b * prm.Ns;
-  const int ns = max(0, min(prm.Ns, N - n0));
-  unsigned long long bar_target = 0;
-  unsigned sweep_no = 0;                                   // parity selects the exchange buffers
+  const int n0 = b * Ns;
+  const int ns = max(0, min(Ns, N - n0));
+  const bool owner = ns > 0;
+  unsigned seq = 0;                                        // sweep number; parity selects the exchange buffers
+  unsigned e1 = 0, e2 = 0, e3 = 0;                         // expected values of the three arrival counters
+  unsigned* const cnt1 = prm.cnt;
+  unsigned* const cnt2 = prm.cnt + 64;
+  unsigned* const cnt3 = prm.cnt + 128;
+  unsigned* status = prm.status;
   int tn = 0;                                              // trace records written (thread 0 of CTA 0)
 
   float* Rb = prm.Rrm + (size_t)m0 * ldr;
   float* Tb = prm.T + m0;
+  // owner-private panels P[slice, 0:k] and W[slice, 0:k] ([Ns][Kpad] floats): shared memory if they fit
+  float* Pc = prm.cache_pw ? reinterpret_cast<float*>(smem + prm.off_pc) : prm.Pown + (size_t)b * Ns * Kpad;
+  float* Wc = prm.cache_pw ? reinterpret_cast<float*>(smem + prm.off_wc) : prm.Wown + (size_t)b * Ns * Kpad;
 
   for (int i = tid; i < prm.Mb; i += kThreads) d_s[i] = 0.f;
-  for (int n = tid; n < ldr; n += kThreads) { p_s[n] = 0.f; pdef_s[n] = 0.f; }
+  for (int n = tid; n < max(ldr, npx); n += kThreads) {
+    if (n < npx) p_s[n] = 0.f;
+    if (n < ldr) pdef_s[n] = 0.f;
+  }
+  if (prm.cache_pw)
+    for (int i = tid; i < Ns * Kpad; i += kThreads) { Pc[i] = 0.f; Wc[i] = 0.f; }
+  for (int i = tid; i < Ns; i += kThreads) praw_s[i] = 0.0;
   __syncthreads();
 
   for (int k = 0; k < K; ++k) {
@@ -349,13 +475,17 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       if (k == 0) sweep_loads<NV, SRC_GLOBAL, DST_NONE, false, true>(prm, Rb, slab, mb, ttil_s, d_s, pdef_s, qs);
       else        sweep_loads<NV, SRC_GLOBAL, DST_GLOBAL, true, true>(prm, Rb, slab, mb, ttil_s, d_s, pdef_s, qs);
     }
+    ++seq;
     {
-      const unsigned buf = sweep_no & 1u;
-      publish_q(prm, qs, prm.Qpart + ((size_t)buf * G + b) * ldr);
+      const unsigned par = seq & 1u;
+      publish_q_ll(prm, qs, prm.Qx + (size_t)par * Gs * G * Ns, b, seq);
       double s = 0.0;
       for (int i = tid; i < mb; i += kThreads) { const double v = (double)ttil_s[i]; s += v * v; }
-      s = block_sum(s, scr);
-      if (tid == 0) prm.Spart[(size_t)buf * G + b] = s;
+      s = block_sum(s, scr);                                                    // (block barriers inside: the q stores are issued)
+      if (tid == 0) {
+        ll_st2d(prm.SBx + ((size_t)par * G + b) * SBw, s, seq);
+        hop_arrive(cnt1);
+      }
     }
     trace_mark(prm, tn, TR_LOADS_DONE);
 
@@ -364,145 +494,180 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
     bool degenerate = false;
     bool first = true;
     for (;;) {
-      const unsigned buf = sweep_no & 1u;
-      const float* Qp = prm.Qpart + (size_t)buf * G * ldr;
-      grid_barrier(prm.bar, bar_target, G);                                   // ---- X1 ----
+      const unsigned par = seq & 1u;
+      // ---- hop 1: |t~|^2 and B (every CTA), raw loads slice (owners) ----
+      e1 += (unsigned)G;
+      hop_wait(cnt1, e1, status);
+      {
+        LLJob jq, jsb;
+        jq.base = prm.Qx + ((size_t)par * Gs + b) * G * Ns; jq.out = praw_s; jq.units = owner ? (Ns >> 1) : 0;
+        jq.nparts = G; jq.stride = Ns; jq.f64_unit0 = false;
+        jsb.base = prm.SBx + (size_t)par * G * SBw; jsb.out = sb_s; jsb.units = 1 + ((gsk && !first) ? ((k + 1) >> 1) : 0);
+        jsb.nparts = G; jsb.stride = SBw; jsb.f64_unit0 = true;
+        ll_reduce2(jsb, jq, seq, status);
+      }
+      __syncthreads();
       trace_mark(prm, tn, TR_X1);
-      const double s = sum_parts(prm.Spart + (size_t)buf * G, G, scr);
-      bool done = false;
-      if (first) {
-        if (!(s > 0.0)) { degenerate = true; break; }                         // zero start column (C7)
-      } else {
-        double bb = 0.0;
-        if (gsk) {                                                            // B = V_(k)^T t~
-          reduce_fparts(B_s, prm.Bpart + (size_t)buf * G * Kpad, k, G, Kpad, scr);
-          double v = 0.0;
-          for (int j = tid; j < k; j += kThreads) v += B_s[j] * B_s[j];
-          bb = block_sum(v, scr);
+      // S7/S8 by warp 0 (fp64 sqrt is a long software sequence: once, not 512 times); meanwhile the owners'
+      // other warps start on p~ = q - W B, which needs only B.
+      if (w == 0) {
+        const double s = sb_s[0];
+        int st = 0;                                                           // 0 continue, 1 done, 2 degenerate
+        double ln = 0.0;
+        if (first) {
+          if (!(s > 0.0)) st = 2;                                             // zero start column (C7)
+        } else {
+          double bb = 0.0;
+          if (gsk) {                                                          // B = V_(k)^T t~
+            for (int j = lane; j < k; j += 32) bb += B_s[j] * B_s[j];
+            bb = warp_sum(bb);
+          }
+          const double l2 = s - bb;                                           // |t~ - V B|^2, V orthonormal
+          if (!(l2 > 0.0)) st = 2;                                            // reading C7
+          else {
+            ln = sqrt(l2);                                                    // S7
+            // S8: listings' strict relative test (reading C3)
+            if ((fabs(lam - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
+          }
         }
-        const double l2 = s - bb;                                             // |t~ - V B|^2, V orthonormal
-        if (!(l2 > 0.0)) { degenerate = true; break; }                        // reading C7
-        lam_new = sqrt(l2);                                                   // S7
-        // S8: listings' strict relative test (reading C3)
-        done = (fabs(lam - lam_new) < prm.eps * lam_new) || (it >= prm.max_iter);
+        if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }
+      }
+      // meanwhile (owners): p~ = q - W B, then the A-partials a_S[j] = sum_{n in S} P[n,j] p~[n] (S3)
+      if (owner && gsk && w > 0) {
+        if (!first) {
+          slice_correct(praw_s, Wc, B_s, ns, k, Kpad, 1);
+          named_bar_sync(1, kThreads - 32);                                   // warps 1..15 (warp 0 is busy with the test)
+        }
+        const int u = tid - 32;                                               // warps 1..15: one thread per pair of A
+        for (int j0 = 2 * u; j0 < k; j0 += 2 * (kThreads - 32)) {
+          double a0 = 0.0, a1 = 0.0;
+          for (int i = 0; i < ns; ++i) {
+            const float2 pj = *reinterpret_cast<const float2*>(Pc + (size_t)i * Kpad + j0);
+            a0 += (double)pj.x * praw_s[i];
+            a1 += (double)pj.y * praw_s[i];
+          }
+          if (j0 + 1 >= k) a1 = 0.0;
+          ll_st2(prm.Ax + ((size_t)par * Gs + b) * Kpad + j0, ll_wordf((float)a0, seq), ll_wordf((float)a1, seq));
+        }
+      }
+      __syncthreads();
+      const int st = reinterpret_cast<const int*>(ctl_s + 1)[0];
+      if (st == 2) { degenerate = true; break; }
+      bool done = false;
+      if (!first) {
+        lam_new = ctl_s[0];
+        done = st == 1;
         if (!done) lam = lam_new;
       }
       trace_mark(prm, tn, TR_TEST);
-      // ---- owners: q_S = sum of the G partials, fixed order, fp64 ----
-      const bool need_q = !done || (gs && k + 1 < K);                         // finalize needs q only for W_k
-      if (ns > 0 && need_q) {
-        const int nsub = min(kThreads / ns, G);
-        const int sub = tid / ns, i = tid - sub * ns;
-        double v = 0.0;
-        if (sub < nsub)
-          for (int bq = sub; bq < G; bq += nsub) v += (double)ld_cg(Qp + (size_t)bq * ldr + n0 + i);
-        if (sub < nsub) scr[sub * ns + i] = v;
-        __syncthreads();
-        if (tid < ns) {
-          double a = 0.0;
-          for (int q = 0; q < nsub; ++q) a += scr[q * ns + tid];
-          praw_s[tid] = a;
-        }
-        __syncthreads();
-        if (gsk && !first) {                                                  // p~ = q - W B
-          const int nsub2 = kThreads / ns;
-          const int sub2 = tid / ns, i2 = tid - sub2 * ns;
-          double c = 0.0;
-          if (sub2 < nsub2) {
-            const float* wr = prm.W + (size_t)(n0 + i2) * Kpad;
-            for (int j = sub2; j < k; j += nsub2) c += (double)ld_cg(wr + j) * B_s[j];
-            scr[sub2 * ns + i2] = c;
-          }
-          __syncthreads();
-          if (tid < ns) {
-            double a = 0.0;
-            for (int q = 0; q < nsub2; ++q) a += scr[q * ns + tid];
-            praw_s[tid] -= a;
-          }
-          __syncthreads();
-        }
-      }
       if (done) break;
       trace_mark(prm, tn, TR_QSLICE);
 
-      if (gsk) {
-        // ---- S3: A-partials a_S[j] = sum_{n in S} P[n,j] p~[n] ----
-        if (ns > 0) {
-          for (int j = tid; j < k; j += kThreads) {
-            const float* pj = prm.P + (size_t)j * N + n0;
-            double a = 0.0;
-            for (int i = 0; i < ns; ++i) a += (double)ld_cg(pj + i) * praw_s[i];
-            prm.Apart[(size_t)b * Kpad + j] = (float)a;
-          }
-        }
+      if (gsk && owner) {
+        if (tid == 0) hop_arrive(cnt2);                                       // A-partials of this pass are out
         trace_mark(prm, tn, TR_APART);
-        grid_barrier(prm.bar, bar_target, G);                                 // ---- X2 ----
-        trace_mark(prm, tn, TR_X2);
-        if (ns > 0) {
-          reduce_fparts(A_s, prm.Apart, k, prm.Gs, Kpad, scr);
-          // p^ = p~ - P_(k) A
-          const int nsub = kThreads / ns;
-          const int sub = tid / ns, i = tid - sub * ns;
-          double c = 0.0;
-          if (sub < nsub) {
-            for (int j = sub; j < k; j += nsub) c += (double)ld_cg(prm.P + (size_t)j * N + n0 + i) * A_s[j];
-            scr[sub * ns + i] = c;
-          }
-          __syncthreads();
-          if (tid < ns) {
-            double a = 0.0;
-            for (int q = 0; q < nsub; ++q) a += scr[q * ns + tid];
-            praw_s[tid] -= a;
-          }
-          __syncthreads();
+        e2 += (unsigned)Gs;
+        hop_wait(cnt2, e2, status);
+        // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
+        {
+          LLJob ja, jn;
+          ja.base = prm.Ax + (size_t)par * Gs * Kpad; ja.out = A_s; ja.units = (k + 1) >> 1; ja.nparts = Gs; ja.stride = Kpad;
+          ja.f64_unit0 = false;
+          jn = ja; jn.units = 0;
+          ll_reduce2(ja, jn, seq, status);
         }
+        __syncthreads();
+        trace_mark(prm, tn, TR_X2);
+        slice_correct(praw_s, Pc, A_s, ns, k, Kpad);
+        __syncthreads();
       }
       // ---- publish the p^ slice and its squared norm (S4, first half) ----
-      if (ns > 0) {
+      if (owner && w == 0) {
         double q2 = 0.0;
-        if (tid < ns) {
-          const float v = (float)praw_s[tid];
-          prm.pvec[n0 + tid] = v;
-          q2 = (double)v * (double)v;
+        for (int u = lane; 2 * u < Ns; u += 32) {
+          const float v0 = (2 * u < ns) ? (float)praw_s[2 * u] : 0.f;
+          const float v1 = (2 * u + 1 < ns) ? (float)praw_s[2 * u + 1] : 0.f;
+          ll_st2(prm.Px + (size_t)par * npx + n0 + 2 * u, ll_wordf(v0, seq), ll_wordf(v1, seq));
+          q2 += (double)v0 * (double)v0 + (double)v1 * (double)v1;
         }
-        q2 = block_sum(q2, scr);
-        if (tid == 0) prm.Npart[b] = q2;
+        q2 = warp_sum(q2);
+        if (lane == 0) {
+          ll_st2d(prm.Nx + ((size_t)par * Gs + b) * 2, q2, seq);
+          hop_arrive(cnt3);                                                   // (the warp's p^ stores precede it in program order)
+        }
       }
       trace_mark(prm, tn, TR_PHAT);
-      grid_barrier(prm.bar, bar_target, G);                                   // ---- X3 ----
+      e3 += (unsigned)Gs;
+      hop_wait(cnt3, e3, status);
+      // ---- hop 3: gather p^ and |p^|^2 ----
+      if (w == kWarps - 1) {
+        LLJob jn;
+        jn.base = prm.Nx + (size_t)par * Gs * 2; jn.out = scr; jn.units = 1; jn.nparts = Gs; jn.stride = 2; jn.f64_unit0 = true;
+        ll_reduce_unit(jn, 0, seq, status);
+        __syncwarp();
+        if (lane == 0) reinterpret_cast<float*>(ctl_s + 2)[0] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+      }
+      {
+        const u64* px = prm.Px + (size_t)par * npx;
+        for (int u0 = tid; 2 * u0 < npx; u0 += kThreads * 4) {
+          u64 x[4], y[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int u = u0 + i * kThreads;
+            x[i] = 0; y[i] = 0;
+            if (2 * u < npx) ll_ld2(px + 2 * u, x[i], y[i]);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int u = u0 + i * kThreads;
+            if (2 * u < npx) {
+              ll_wait2(px + 2 * u, seq, x[i], y[i], status);
+              *reinterpret_cast<float2*>(p_s + 2 * u) = make_float2(ll_f(x[i]), ll_f(y[i]));
+            }
+          }
+        }
+      }
+      __syncthreads();
       trace_mark(prm, tn, TR_X3);
-      const double pn2 = sum_parts(prm.Npart, prm.Gs, scr);
-      if (!(pn2 > 0.0)) { degenerate = true; break; }                         // reading C7
-      const float inv_pn = (float)(1.0 / sqrt(pn2));                          // p = p^/|p^|
-      for (int n = tid; n < ldr; n += kThreads) p_s[n] = (n < N) ? ld_cg(prm.pvec + n) * inv_pn : 0.f;
+      const float inv_pn = reinterpret_cast<const float*>(ctl_s + 2)[0];      // p = p^/|p^|
+      if (!(inv_pn > 0.f)) { degenerate = true; break; }                      // reading C7
+      for (int n = tid; n < npx; n += kThreads) p_s[n] *= inv_pn;             // each thread rescales what it wrote
       __syncthreads();
       first = false;
       trace_mark(prm, tn, TR_PREADY);
       // ---- FUSED sweep: t~ = R p (S5), q = R^T t~, s = |t~|^2 ----
-      ++sweep_no;
+      ++seq;
       ++it;
       {
-        const unsigned nbuf = sweep_no & 1u;
-        const bool rev = (sweep_no & 1u) != 0;
+        const unsigned npar = seq & 1u;
+        const bool rev = (seq & 1u) != 0;
         if constexpr (RESIDENT) sweep_fused<NV, SRC_SLAB>(prm, Rb, slab, mb, p_s, ttil_s, qs, red_s, sgrp, false);
         else                    sweep_fused<NV, SRC_GLOBAL>(prm, Rb, slab, mb, p_s, ttil_s, qs, red_s, sgrp, rev);
         trace_mark(prm, tn, TR_SWEEP);
-        publish_q(prm, qs, prm.Qpart + ((size_t)nbuf * G + b) * ldr);
+        publish_q_ll(prm, qs, prm.Qx + (size_t)npar * Gs * G * Ns, b, seq);
+        u64* sbx = prm.SBx + ((size_t)npar * G + b) * SBw;
         if (tid == 0) {
           double a = 0.0;
           for (int g = 0; g < NG; ++g) a += sgrp[g];
-          prm.Spart[(size_t)nbuf * G + b] = a;
+          ll_st2d(sbx, a, seq);
         }
         if (gsk) {                                                            // S6: B-partials V^T t~
-          float* bp = prm.Bpart + ((size_t)nbuf * G + b) * Kpad;
-          for (int j = w; j < k; j += kWarps) {
-            const float* vj = Tb + (size_t)j * M;
-            float a = 0.f;
-            for (int i = lane; i < mb; i += 32) a = fmaf(ld_cg(vj + i), ttil_s[i], a);
-            const double sj = warp_sum((double)a);
-            if (lane == 0) bp[j] = (float)sj;
+          for (int j0 = 2 * w; j0 < k; j0 += 2 * kWarps) {
+            const float* v0 = Tb + (size_t)j0 * M;
+            const float* v1 = v0 + M;
+            const bool two = j0 + 1 < k;
+            float a0 = 0.f, a1 = 0.f;
+            for (int i = lane; i < mb; i += 32) {
+              const float tt = ttil_s[i];
+              a0 = fmaf(v0[i], tt, a0);
+              if (two) a1 = fmaf(v1[i], tt, a1);
+            }
+            const double s0 = warp_sum((double)a0), s1 = warp_sum((double)a1);
+            if (lane == 0) ll_st2(sbx + 2 + j0, ll_wordf((float)s0, seq), ll_wordf((float)s1, seq));
           }
         }
+        __syncthreads();                                                      // all LL stores of this CTA are issued
+        if (tid == 0) hop_arrive(cnt1);
         trace_mark(prm, tn, TR_PUBLISHED);
       }
     }
@@ -510,10 +675,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
     // ---- component done ----
     if (degenerate) {
       for (int i = tid; i < mb; i += kThreads) { Tb[(size_t)k * M + i] = 0.f; d_s[i] = 0.f; }
-      if (tid < ns) {
-        prm.P[(size_t)k * N + n0 + tid] = 0.f;
-        prm.W[(size_t)(n0 + tid) * Kpad + k] = 0.f;
-      }
+      if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = 0.f;
+      if (tid < Ns) { Pc[(size_t)tid * Kpad + k] = 0.f; Wc[(size_t)tid * Kpad + k] = 0.f; }
       for (int n = tid; n < ldr; n += kThreads) pdef_s[n] = 0.f;
       if (b == 0 && tid == 0) { prm.lambda[k] = 0.f; prm.iters[k] = 0; }
       if (tid == 0) lam_s[k] = 0.f;
@@ -525,7 +688,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         float t = ttil_s[i];
         if (gsk) {
           float corr = 0.f;
-          for (int j = 0; j < k; ++j) corr = fmaf(ld_cg(Tb + (size_t)j * M + i), (float)B_s[j], corr);
+          for (int j = 0; j < k; ++j) corr = fmaf(Tb[(size_t)j * M + i], (float)B_s[j], corr);
           t -= corr;
         }
         d_s[i] = t;                                                           // R -= lambda v p^T  /  R -= t p^T
@@ -534,14 +697,14 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       if (tid < ns) {
         const float pk = p_s[n0 + tid];
         prm.P[(size_t)k * N + n0 + tid] = pk;
+        Pc[(size_t)tid * Kpad + k] = pk;
         if (gs && k + 1 < K)                                                  // W_k = R_(k+1)^T v_k
-          prm.W[(size_t)(n0 + tid) * Kpad + k] = (float)(praw_s[tid] / lam_new - lam_new * (double)pk);
+          Wc[(size_t)tid * Kpad + k] = (float)(praw_s[tid] / lam_new - lam_new * (double)pk);
       }
-      for (int n = tid; n < ldr; n += kThreads) pdef_s[n] = p_s[n];
+      for (int n = tid; n < ldr; n += kThreads) pdef_s[n] = (n < npx) ? p_s[n] : 0.f;
       if (b == 0 && tid == 0) { prm.lambda[k] = lamf; prm.iters[k] = it; }
       if (tid == 0) lam_s[k] = lamf;
     }
-    ++sweep_no;                                                               // next LOADS sweep takes the other buffers
     __syncthreads();
     trace_mark(prm, tn, TR_FINAL);
   }

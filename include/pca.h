@@ -56,10 +56,14 @@ enum {
 /* Options for pca_set_option (all optional; defaults are chosen by pca_create). */
 enum {
   PCA_OPT_PATH = 1,     /* 0 = auto; two-sweep kernel: 1 = HBM-streaming, 2 = SMEM-resident;
-                           single-sweep kernel (R read once per inner pass): 3 = streaming, 4 = resident */
+                           single-sweep kernel (R read once per inner pass): 3 = streaming, 4 = SMEM-resident,
+                           5 = register-resident (4*M*N up to ~19 MB on 148 SMs) */
   PCA_OPT_CTAS = 2,     /* number of CTAs of the persistent kernel (0 = auto) */
   PCA_OPT_CENTER_MODE = 3, /* 0 = column means (default), 1 = literal eq. (1) mean column */
-  PCA_OPT_TRACE = 4     /* single-sweep kernel only: capacity (records) of the device-side phase trace, 0 = off
+  PCA_OPT_OWNERS = 5,   /* register-resident kernel: number of slice-owner CTAs (0 = auto; rounded down to a power of two) */
+  PCA_OPT_KDIRECT = 6,  /* register-resident kernel: the Gram-Schmidt coefficients B of component k are combined in two
+                           levels for k > this value (-1 = default) */
+  PCA_OPT_TRACE = 4     /* single-sweep kernels only: capacity (records) of the device-side phase trace, 0 = off
                            (default).  See pca_trace. */
 };
 
@@ -83,7 +87,8 @@ enum {
 
 /* Fields for pca_get_info. */
 enum {
-  PCA_INFO_PATH = 1,        /* 1, 2 = two-sweep kernel streaming / resident; 3, 4 = single-sweep kernel streaming / resident */
+  PCA_INFO_PATH = 1,        /* 1, 2 = two-sweep kernel streaming / resident; 3, 4 = single-sweep kernel streaming / resident;
+                               5 = register-resident single-sweep kernel */
   PCA_INFO_CTAS = 2,        /* CTAs of the persistent solve kernel */
   PCA_INFO_THREADS = 3,     /* threads per CTA */
   PCA_INFO_SMEM_BYTES = 4,  /* dynamic shared memory per CTA */
@@ -91,6 +96,7 @@ enum {
   PCA_INFO_LAUNCHES_PER_RUN = 6, /* kernel launches one pca_run enqueues */
   PCA_INFO_NUM_SMS = 7,
   PCA_INFO_ROW_GROUP_THREADS = 8, /* single-sweep kernel: threads that share one row of R (0 otherwise) */
+  PCA_INFO_OWNERS = 10,     /* slice-owner CTAs (CTAs that combine the partial loads of a column slice) */
   PCA_INFO_RUN_STATUS = 9   /* SYNCHRONISES the device and reads the status word of the last pca_run: 0 = ok,
                                1 = a cross-CTA exchange wait gave up (results invalid; never in a correct run) */
 };

@@ -14,9 +14,11 @@
 
 #include "pca_center.cuh"
 #include "pca_fused.cuh"
+#include "pca_reg.cuh"
 #include "pca_solve.cuh"
 
 using pca::FusedParams;
+using pca::RegParams;
 using pca::SolveParams;
 
 namespace {
@@ -50,6 +52,20 @@ const FusedVariant kFusedVariants[] = {
 
 }  // namespace
 
+namespace pca {
+reg_kernel_t reg_kernel_lookup_part0(int gt, int rpt);
+reg_kernel_t reg_kernel_lookup_part1(int gt, int rpt);
+reg_kernel_t reg_kernel_lookup_part2(int gt, int rpt);
+reg_kernel_t reg_kernel_lookup_part3(int gt, int rpt);
+reg_kernel_t reg_kernel_lookup(int gt, int rpt) {
+  reg_kernel_t f = reg_kernel_lookup_part0(gt, rpt);
+  if (!f) f = reg_kernel_lookup_part1(gt, rpt);
+  if (!f) f = reg_kernel_lookup_part2(gt, rpt);
+  if (!f) f = reg_kernel_lookup_part3(gt, rpt);
+  return f;
+}
+}  // namespace pca
+
 struct pca_ctx {
   long long M = 0, N = 0;
   int K = 0;
@@ -59,10 +75,15 @@ struct pca_ctx {
   // device
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
-  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0;
+  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1;
   // plan
   bool planned = false;
-  int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel)
+  int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
+                 // 5 register-resident single-sweep kernel
+  pca::reg_kernel_t rfn = nullptr;
+  RegParams rprm{};
+  int r_gt = 0, r_rpt = 0;
+  size_t ws_off_bx = 0;
   const Variant* variant = nullptr;
   SolveParams prm{};
   const FusedVariant* fvariant = nullptr;
@@ -257,8 +278,109 @@ int make_fused_plan(pca_ctx* c, int want) {
   return PCA_OK;
 }
 
+// Register-resident single-sweep kernel (pca_reg.cuh): GT threads share a row, 8 columns per thread, RPT rows per
+// row group, the whole row block of a CTA in registers.  Fits when ceil(M/G) <= (512/GT)*7 with G <= #SMs.
+int make_reg_plan(pca_ctx* c) {
+  const long long M = c->M, N = c->N;
+  const int sms = c->num_sms;
+  int GT = 8;
+  while (8LL * GT < N) GT *= 2;
+  if (GT > pca::kThreads) return PCA_EUNSUPPORTED;
+  const int NG = pca::kThreads / GT, ldr = 8 * GT;
+  int G = c->opt_ctas > 0 ? c->opt_ctas : (int)ceil_div(M, (long long)NG * 7);
+  if (G < 1) G = 1;
+  if (G > sms) return PCA_EUNSUPPORTED;
+  const int Mb = (int)ceil_div(M, G);
+  int RPT = 0;
+  for (int r : {2, 4, 7})
+    if ((long long)NG * r >= Mb) { RPT = r; break; }
+  if (!RPT) return PCA_EUNSUPPORTED;
+  pca::reg_kernel_t fn = pca::reg_kernel_lookup(GT, RPT);
+  if (!fn) return PCA_EUNSUPPORTED;
+  int g2 = 1;
+  while (g2 * 2 <= G) g2 *= 2;                                       // owners: a power of two <= G
+  RegParams p{};
+  p.G = G; p.Mb = Mb; p.ldr = ldr; p.Kpad = (int)round_up(c->K, 4);
+  const bool gs = c->algo == PCA_ALGO_GS;
+  size_t smem = 0;
+  auto carve_reg = [&](int Gs) -> size_t {
+    p.Gs = Gs; p.Ns = ldr / Gs;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 16); return (int)o; };
+    const size_t rows = (size_t)NG * RPT;
+    p.off_p = take((size_t)2 * ldr * 4);
+    p.off_ttil = take(rows * 4);
+    p.off_d = take(rows * 4);
+    p.off_qs = take((size_t)NG * ldr * 4);
+    p.off_red = take((size_t)pca::kThreads * 4);
+    p.off_sgrp = take((size_t)NG * 8);
+    p.off_B = take((size_t)(4 + p.Kpad) * 8);
+    p.off_A = take((size_t)(2 + p.Kpad) * 8);
+    p.off_scr = take((size_t)pca::kThreads * 8);
+    p.off_praw = take((size_t)2 * p.Ns * 8);
+    p.off_bred = take((size_t)pca::kThreads * 4);
+    const size_t KV = (size_t)(p.Kpad | 1);                           // odd row stride (bank-conflict-free both ways)
+    p.off_vb = take(gs ? rows * KV * 4 : 0);
+    p.off_pc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
+    p.off_wc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
+    return off;
+  };
+  int Gs = c->opt_owners > 0 ? c->opt_owners : 32;
+  if (Gs > g2) Gs = g2;
+  if (Gs > ldr / 2) Gs = ldr / 2;
+  int gq = 1;
+  while (gq * 2 <= Gs) gq *= 2;
+  Gs = gq;
+  for (;;) {
+    smem = carve_reg(Gs);
+    if (smem <= (size_t)c->smem_optin) break;
+    if (Gs * 2 > g2 || Gs * 2 > ldr / 2) return PCA_EUNSUPPORTED;   // more owners = smaller P / W panels per owner
+    Gs *= 2;
+  }
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, pca::kThreads, smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  if ((long long)per_sm * sms < G) return PCA_EUNSUPPORTED;
+
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  p.kdirect = c->opt_kdirect >= 0 ? (c->opt_kdirect > 30 ? 30 : c->opt_kdirect) : 0;    // direct: <= 16 units, one per warp
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
+  take((size_t)M * (size_t)N * 4);                                   // residual of eq. (4), column-major (ABI layout)
+  c->ws_off_rrm = take((size_t)M * (size_t)ldr * 4);                 // row-major copy: read once, written once
+  c->ws_off_xchg = off;
+  c->ws_off_qx = take((size_t)2 * G * ldr * 8);
+  c->ws_off_sbx = take((size_t)2 * G * (2 + p.Kpad) * 8);
+  c->ws_off_bx = take((size_t)2 * (2 + p.Kpad) * 2 * 8);
+  c->ws_off_ax = take((size_t)2 * p.Gs * p.Kpad * 8);
+  c->ws_off_px = take((size_t)2 * ldr * 8);
+  c->ws_off_nx = take((size_t)2 * p.Gs * 8 * 8);
+  c->ws_off_status = take(256);
+  c->ws_xchg_bytes = off - c->ws_off_xchg;
+  c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1) * 8 : 0);
+  p.trace_cap = c->opt_trace;
+  c->ws_bytes = off;
+  c->rprm = p;
+  c->rfn = fn;
+  c->r_gt = GT; c->r_rpt = RPT;
+  c->smem_bytes = smem;
+  c->path = 5;
+  c->planned = true;
+  c->ws = nullptr;
+  c->ws_given = 0;
+  c->ran = false;
+  return PCA_OK;
+}
+
 int make_plan(pca_ctx* c) {
   c->planned = false;
+  if (c->opt_path == 0 || c->opt_path == 5) {
+    const int rc = make_reg_plan(c);
+    if (rc == PCA_OK || c->opt_path != 0) return rc;
+    if (rc == PCA_ECUDA) return rc;
+  }
   if (c->opt_path == 0 || c->opt_path == 3 || c->opt_path == 4) {
     const int rc = make_fused_plan(c, c->opt_path);
     if (rc == PCA_OK || c->opt_path != 0) return rc;
@@ -371,7 +493,7 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
   if (!c) return PCA_EINVAL;
   switch (option) {
     case PCA_OPT_PATH:
-      if (value < 0 || value > 4) return PCA_EINVAL;
+      if (value < 0 || value > 5) return PCA_EINVAL;
       c->opt_path = (int)value;
       break;
     case PCA_OPT_CTAS:
@@ -382,6 +504,14 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
       if (value < 0 || value > 1) return PCA_EINVAL;
       c->opt_center_mode = (int)value;
       return PCA_OK;
+    case PCA_OPT_OWNERS:
+      if (value < 0 || value > c->num_sms) return PCA_EINVAL;
+      c->opt_owners = (int)value;
+      break;
+    case PCA_OPT_KDIRECT:
+      if (value < -1 || value > (1 << 30)) return PCA_EINVAL;
+      c->opt_kdirect = (int)value;
+      break;
     case PCA_OPT_TRACE:
       if (value < 0 || value > (1 << 24)) return PCA_EINVAL;
       c->opt_trace = (int)value;
@@ -396,12 +526,13 @@ int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
   if (!c || !value || !c->planned) return PCA_EINVAL;
   switch (field) {
     case PCA_INFO_PATH: *value = c->path; break;
-    case PCA_INFO_CTAS: *value = c->path >= 3 ? c->fprm.G : c->prm.G; break;
+    case PCA_INFO_CTAS: *value = c->path == 5 ? c->rprm.G : (c->path >= 3 ? c->fprm.G : c->prm.G); break;
+    case PCA_INFO_OWNERS: *value = c->path == 5 ? c->rprm.Gs : (c->path >= 3 ? c->fprm.Gs : c->prm.Gs); break;
     case PCA_INFO_THREADS: *value = pca::kThreads; break;
     case PCA_INFO_SMEM_BYTES: *value = (int64_t)c->smem_bytes; break;
-    case PCA_INFO_ROWS_PER_CTA: *value = c->path >= 3 ? c->fprm.Mb : c->prm.Mb; break;
+    case PCA_INFO_ROWS_PER_CTA: *value = c->path == 5 ? c->rprm.Mb : (c->path >= 3 ? c->fprm.Mb : c->prm.Mb); break;
     case PCA_INFO_LAUNCHES_PER_RUN: *value = c->path >= 3 ? 3 : 1; break;
-    case PCA_INFO_ROW_GROUP_THREADS: *value = c->path >= 3 ? c->fprm.GT : 0; break;
+    case PCA_INFO_ROW_GROUP_THREADS: *value = c->path == 5 ? c->r_gt : (c->path >= 3 ? c->fprm.GT : 0); break;
     case PCA_INFO_NUM_SMS: *value = c->num_sms; break;
     case PCA_INFO_RUN_STATUS: {
       *value = 0;
@@ -451,6 +582,33 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
   if (!c->ws || c->ws_given < c->ws_bytes) return PCA_EWORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   unsigned char* ws = static_cast<unsigned char*>(c->ws);
+  if (c->path == 5) {
+    RegParams p = c->rprm;
+    p.Rrm = reinterpret_cast<float*>(ws + c->ws_off_rrm);
+    p.T = T; p.P = P; p.lambda = lambda; p.iters = iters;
+    typedef unsigned long long u64;
+    p.Qx = reinterpret_cast<u64*>(ws + c->ws_off_qx);
+    p.SBx = reinterpret_cast<u64*>(ws + c->ws_off_sbx);
+    p.Bx = reinterpret_cast<u64*>(ws + c->ws_off_bx);
+    p.Ax = reinterpret_cast<u64*>(ws + c->ws_off_ax);
+    p.Px = reinterpret_cast<u64*>(ws + c->ws_off_px);
+    p.Nx = reinterpret_cast<u64*>(ws + c->ws_off_nx);
+    p.status = reinterpret_cast<unsigned*>(ws + c->ws_off_status);
+    p.trace = reinterpret_cast<unsigned long long*>(ws + c->ws_off_trace);
+    PCA_CUDA(c, cudaMemsetAsync(ws + c->ws_off_xchg, 0, c->ws_xchg_bytes, st));   // sequence numbers start at 0
+    if (p.trace_cap > 0) PCA_CUDA(c, cudaMemsetAsync(p.trace, 0, 8, st));
+    const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
+    pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X
+    PCA_CUDA(c, cudaGetLastError());
+    void* rargs[] = {&p};
+    PCA_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(c->rfn), dim3((unsigned)p.G), dim3(pca::kThreads),
+                                            rargs, c->smem_bytes, st));
+    const dim3 ogrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(c->N, 32));
+    pca::pca_transpose_plain_kernel<<<ogrid, 256, 0, st>>>(p.Rrm, reinterpret_cast<float*>(ws), c->M, p.N, p.ldr);
+    PCA_CUDA(c, cudaGetLastError());
+    c->ran = true;
+    return PCA_OK;
+  }
   if (c->path >= 3) {
     FusedParams p = c->fprm;
     p.Rrm = reinterpret_cast<float*>(ws + c->ws_off_rrm);

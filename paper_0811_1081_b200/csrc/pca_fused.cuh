@@ -724,7 +724,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
 
 // ------------------------------------------------------------------------------------ transposes
 // Rrm[m][n] = X[n*M + m] for n < N, 0 for N <= n < ldr                      (R <- X)
-__global__ void __launch_bounds__(256) pca_transpose_in_kernel(const float* __restrict__ X, float* __restrict__ Rrm,
+static __global__ void __launch_bounds__(256) pca_transpose_in_kernel(const float* __restrict__ X, float* __restrict__ Rrm,
                                                                long long M, int N, int ldr) {
   __shared__ float tile[32][33];
   const long long mt = (long long)blockIdx.x * 32;
@@ -747,7 +747,7 @@ __global__ void __launch_bounds__(256) pca_transpose_in_kernel(const float* __re
 
 // Rout[n*M + m] = Rrm[m][n] - d[m]*p[n]: the residual of eq. (4) in the ABI's column-major layout,
 // with the last component's deflation (d = T[:,K-1] after the epilogue, p = P[:,K-1]) applied.
-__global__ void __launch_bounds__(256) pca_transpose_out_kernel(const float* __restrict__ Rrm, float* __restrict__ Rout,
+static __global__ void __launch_bounds__(256) pca_transpose_out_kernel(const float* __restrict__ Rrm, float* __restrict__ Rout,
                                                                 const float* __restrict__ d, const float* __restrict__ p,
                                                                 long long M, int N, int ldr) {
   __shared__ float tile[32][33];

@@ -93,6 +93,18 @@ SMALL_CASES = [
     (3, 8192, 256, 16, 1, 0),       # tall: more than one row chunk per CTA on the streaming plan
     (4, 1024, 64, 64, 0, 0),        # K = N full decomposition
     (1, 64, 300, 4, 0, 0),          # M < N (the paper assumes N <= M; accepted anyway)
+    # register-resident single-sweep kernel (path 5; also what the auto plan picks for all the small cases above)
+    (0, 256, 64, 8, 5, 0),          # one CTA, 8 threads per row
+    (0, 256, 64, 8, 5, 6),          # ... 6 CTAs, 4 owners
+    (1, 1000, 200, 6, 5, 0),        # 32 threads per row, 9 CTAs (ragged last row block)
+    (1, 1000, 200, 6, 5, 40),       # ... 40 CTAs x 25 rows
+    (1, 1027, 131, 5, 5, 0),        # M % 4 != 0 and N % 4 != 0 (zero-padded columns)
+    (1, 3000, 700, 12, 5, 0),       # 128 threads per row (cross-warp row reduction), 108 CTAs
+    (2, 2048, 512, 20, 5, 0),       # collinear columns; two-level combination of B
+    (3, 8192, 256, 16, 5, 0),       # tall
+    (4, 1024, 64, 64, 5, 0),        # K = N full decomposition, 3 CTAs
+    (1, 64, 300, 4, 5, 0),          # M < N
+    (1, 1024, 4096, 6, 5, 0),       # 512 threads per row (one row group per CTA)
 ]
 
 
@@ -123,8 +135,8 @@ def test_paths_agree_and_are_deterministic(binding):
     each plan is bitwise reproducible run to run (fixed-order reductions)."""
     cfg = inputs.scaled(inputs.config(1), 1536, 384, K=6)
     pr = inputs.generate(cfg)
-    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2, 3, 3, 4, 4)]
-    for a, b in ((0, 1), (2, 3), (4, 5), (6, 7)):
+    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2, 3, 3, 4, 4, 5, 5)]
+    for a, b in ((0, 1), (2, 3), (4, 5), (6, 7), (8, 9)):
         for key in ("T", "P", "lam", "iters"):
             np.testing.assert_array_equal(runs[a][key], runs[b][key])
     for r in runs[1:]:
@@ -138,7 +150,7 @@ def test_eps_zero_runs_exactly_max_iter(binding):
     cfg = inputs.scaled(inputs.config(0), 256, 64, K=3)
     pr = inputs.generate(cfg)
     for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
-        for path in (0, 1, 2, 3, 4):
+        for path in (0, 1, 2, 3, 4, 5):
             got = binding.fit(pr.X, 3, 0.0, 7, algo, path=path)
             assert got["iters"].tolist() == [7, 7, 7]
         got = binding.fit(pr.X, 3, 0.0, 1, algo)               # a single pass per component

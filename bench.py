@@ -194,8 +194,8 @@ def roofline(prob, run_ms_mean, peaks):
     total_iters = int(iters.sum())
     return {
         "bound": "hbm",
-        "kernel": ("pca_fused_kernel" if single else "pca_solve_kernel") +
-                  " (persistent; all passes of all components in one launch)",
+        "kernel": (("pca_reg_kernel" if "register" in prob.ctx.info()["path"] else "pca_fused_kernel") if single
+                   else "pca_solve_kernel") + " (persistent; all passes of all components in one launch)",
         "achieved": round(achieved, 1), "peak": peak, "peak_source": peaks["source"], "unit": "GB/s",
         "frac": round(achieved / peak, 4), "traffic": peaks.get("traffic"),
         "algorithmic_bytes_per_launch": int(nbytes), "inner_iterations_per_launch": total_iters,

@@ -210,6 +210,23 @@ def roofline(prob, run_ms_mean, peaks):
     }, iters
 
 
+def max_over_ranks(x, world, device):
+    """Replicas only: the job's time is the slowest rank's.  The ONLY collective of the
+    benchmark (a scalar), not of the data path; works on any backend (nccl on GPUs, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def aggregate_value(K, world, ms_per_step):
+    """Whole-job throughput of `world` independent replicas of a K-component solve."""
+    return world * K / (ms_per_step * 1e-3)
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -301,12 +318,9 @@ def run_cuda_arm(args):
     clocks = sampler.stop()
     step_ms = float(np.sum([e[0].elapsed_time(e[1]) for e in evs]))
     run_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
-    if world > 1:
-        tt = torch.tensor([step_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        step_ms = float(tt.item())
+    step_ms = max_over_ranks(step_ms, world, "cuda")
     ms_per_step = step_ms / args.steps
-    value = world * K / (ms_per_step * 1e-3)
+    value = aggregate_value(K, world, ms_per_step)
     roof, iters = roofline(prob, run_ms, peaks)
 
     out = None
@@ -334,10 +348,7 @@ def run_cuda_arm(args):
     # ---- e2e: host buffers through pca_fit_host (every rank, max over ranks) ----
     if not args.no_e2e:
         dt, h2d, d2h = e2e_leg(prob, pr.X, max(1, min(args.steps, args.e2e_steps)))
-        if world > 1:
-            tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
+        dt = max_over_ranks(dt, world, "cuda")
         if rank == 0:
             out["e2e"] = {"value": round(world * K / dt, 3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                           "d2h_bytes_per_step": d2h, "ms_per_step": round(dt * 1e3, 3),

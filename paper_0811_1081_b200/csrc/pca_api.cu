@@ -323,6 +323,11 @@ int make_reg_plan(pca_ctx* c) {
     p.off_vb = take(gs ? rows * KV * 4 : 0);
     p.off_pc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
     p.off_wc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
+    p.off_x = -1;
+    if (G == 1) {                                                     // one CTA: exchange buffers in shared memory if they fit
+      const size_t xwords = (size_t)4 * ldr + 4 * (1 + p.Kpad / 2) + 4 * (2 + p.Kpad) + 4 * (p.Kpad / 2) + 2 * (Gs * 2 + 4);
+      if (off + xwords * 8 <= (size_t)c->smem_optin) p.off_x = take(xwords * 8);
+    }
     return off;
   };
   int Gs = c->opt_owners > 0 ? c->opt_owners : 32;

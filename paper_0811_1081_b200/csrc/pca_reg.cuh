@@ -57,6 +57,7 @@ struct RegParams {
   int trace_cap;
   // shared-memory carve-up (byte offsets)
   int off_p, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_bred, off_vb, off_pc, off_wc;
+  int off_x;             // >= 0 (one CTA only): the exchange buffers live in shared memory at this offset
 };
 
 // ------------------------------------------------------------------------------------ trace
@@ -74,6 +75,28 @@ __device__ __forceinline__ void reg_trace(const RegParams& prm, int& tn, int pha
       prm.trace[1 + (size_t)blockIdx.x * capb + tn] = ((unsigned long long)phase << 56) | (c & 0x00ffffffffffffffULL);
       ++tn;
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------ LL words, generic addresses
+// Same protocol as pca_fused.cuh ("LL exchange"), but through GENERIC addresses: when the whole problem runs in ONE CTA
+// the exchange buffers are placed in shared memory (the warps of the CTA exchange through them exactly as CTAs do through
+// L2, at shared-memory latency), otherwise they are the global buffers of the workspace.
+__device__ __forceinline__ void gl_st2(u64* p, u64 a, u64 b) {
+  asm volatile("st.relaxed.gpu.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ void gl_ld2(const u64* p, u64& a, u64& b) {
+  asm volatile("ld.relaxed.gpu.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void gl_st2d(u64* p, double v, unsigned seq) {
+  const u64 bits = (u64)__double_as_longlong(v);
+  gl_st2(p, ll_word((unsigned)bits, seq), ll_word((unsigned)(bits >> 32), seq));
+}
+__device__ __forceinline__ void gl_wait2(const u64* p, unsigned seq, u64& a, u64& b, unsigned* status) {
+  unsigned spins = 0;
+  while ((unsigned)(a >> 32) != seq || (unsigned)(b >> 32) != seq) {
+    gl_ld2(p, a, b);
+    if (++spins > kSpinLimit) { *status = 1u; break; }
   }
 }
 
@@ -235,13 +258,13 @@ __device__ __forceinline__ void reg_ll_unit(const u64* base, int stride, int npa
     for (int i = 0; i < PL; ++i) {
       const int bq = b0 + 32 * i;
       x[i] = 0; y[i] = 0;
-      if (bq < nparts) ll_ld2(base + (size_t)bq * stride + 2 * u, x[i], y[i]);
+      if (bq < nparts) gl_ld2(base + (size_t)bq * stride + 2 * u, x[i], y[i]);
     }
 #pragma unroll
     for (int i = 0; i < PL; ++i) {
       const int bq = b0 + 32 * i;
       if (bq < nparts) {
-        ll_wait2(base + (size_t)bq * stride + 2 * u, seq, x[i], y[i], status);
+        gl_wait2(base + (size_t)bq * stride + 2 * u, seq, x[i], y[i], status);
         if (f64) a0 += ll_d(x[i], y[i]);
         else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
       }
@@ -260,7 +283,7 @@ __device__ __forceinline__ void reg_ll_units4(const u64* base, int stride, int u
   for (int i = 0; i < 4; ++i) {
     const int u = u0 + i * ustep;
     x[i] = 0; y[i] = 0;
-    if (u < units && lane < nparts) ll_ld2(base + (size_t)lane * stride + (size_t)u * ustride, x[i], y[i]);
+    if (u < units && lane < nparts) gl_ld2(base + (size_t)lane * stride + (size_t)u * ustride, x[i], y[i]);
   }
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -268,7 +291,7 @@ __device__ __forceinline__ void reg_ll_units4(const u64* base, int stride, int u
     if (u < units) {                                                    // warp-uniform
       double a0 = 0.0, a1 = 0.0;
       if (lane < nparts) {
-        ll_wait2(base + (size_t)lane * stride + (size_t)u * ustride, seq, x[i], y[i], status);
+        gl_wait2(base + (size_t)lane * stride + (size_t)u * ustride, seq, x[i], y[i], status);
         a0 = (double)ll_f(x[i]); a1 = (double)ll_f(y[i]);
       }
       a0 = warp_sum(a0);
@@ -316,7 +339,7 @@ __device__ __forceinline__ void reg_gather_issue(const RegGather& gq, u64 (&x)[I
   for (int i = 0; i < INF; ++i) {
     const int part = pslot + i * pstep;
     x[i] = 0; y[i] = 0;
-    if (part < gq.nparts && pair < gq.npairs) ll_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
+    if (part < gq.nparts && pair < gq.npairs) gl_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
   }
 }
 
@@ -332,14 +355,14 @@ __device__ __forceinline__ void reg_gather_finish(const RegGather& gq, u64 (&x)[
     for (int i = 0; i < INF; ++i) {
       const int part = pslot + i * pstep;
       if (part < gq.nparts) {
-        ll_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
+        gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
         if (f64) a0 += ll_d(x[i], y[i]);
         else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
       }
     }
     for (int part = pslot + INF * pstep; part < gq.nparts; part += pstep) {   // more parts than INF rounds cover (rare)
       u64 xx = 0, yy = 0;
-      ll_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, xx, yy, status);
+      gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, xx, yy, status);
       if (f64) a0 += ll_d(xx, yy);
       else { a0 += (double)ll_f(xx); a1 += (double)ll_f(yy); }
     }
@@ -381,7 +404,7 @@ __device__ __forceinline__ void reg_publish_q(const RegParams& prm, const float*
       a.x += v.x; a.y += v.y;
     }
     const int o = c / Ns, i = c - o * Ns;
-    ll_st2(Qpar + ((size_t)o * prm.G + b) * Ns + i, ll_wordf(a.x, seq), ll_wordf(a.y, seq));
+    gl_st2(Qpar + ((size_t)o * prm.G + b) * Ns + i, ll_wordf(a.x, seq), ll_wordf(a.y, seq));
   }
 }
 
@@ -394,7 +417,7 @@ __device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const fl
   if (tid == 0) {
     double a = 0.0;
     for (int g = 0; g < NG; ++g) a += sgrp[g];
-    ll_st2d(sbx, a, seq);
+    gl_st2d(sbx, a, seq);
   }
   if (!with_b) return;
   int Kc = 32;
@@ -407,18 +430,23 @@ __device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const fl
   for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   const float nb = __shfl_down_sync(0xffffffffu, a, parts);             // column j + 1 (same part)
   if (part == 0 && (j & 1) == 0 && j < k)
-    ll_st2(sbx + (size_t)(1 + (j >> 1)) * G * 2, ll_wordf(a, seq), ll_wordf(j + 1 < k ? nb : 0.f, seq));
+    gl_st2(sbx + (size_t)(1 + (j >> 1)) * G * 2, ll_wordf(a, seq), ll_wordf(j + 1 < k ? nb : 0.f, seq));
 }
 
-// praw[i] -= sum_{j<k} C[i*KP + j] * coef[j] for the ns columns of this owner (one warp per column, all warps).
+// praw[i] -= sum_{j<k} C[i*KP + j] * coef[j] for the ns columns of this owner: LPR lanes per column (8 for k <= 64, else 32;
+// lane l takes j = l, l + LPR, ... in order, then a shuffle tree), 32/LPR columns per warp and round.
 __device__ __forceinline__ void reg_slice_correct(double* praw_s, const float* C, int KP, const double* coef_s, int ns, int k) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  for (int i = w; i < ns; i += kWarps) {
-    const float* ci = C + (size_t)i * KP;
+  const int lpr = k <= 64 ? 8 : 32, rpw = 32 / lpr, ll = lane & (lpr - 1);
+  for (int i0 = 0; i0 < ns; i0 += rpw * kWarps) {                             // (uniform trip count: shuffles inside)
+    const int i = i0 + w * rpw + lane / lpr;
     double c = 0.0;
-    for (int j = lane; j < k; j += 32) c += (double)ci[j] * coef_s[j];
-    c = warp_sum(c);
-    if (lane == 0) praw_s[i] -= c;
+    if (i < ns) {
+      const float* ci = C + (size_t)i * KP;
+      for (int j = ll; j < k; j += lpr) c += (double)ci[j] * coef_s[j];
+    }
+    for (int o = lpr >> 1; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if (ll == 0 && i < ns) praw_s[i] -= c;
   }
 }
 
@@ -436,18 +464,7 @@ __device__ __forceinline__ void reg_publish_a(const float* Pc, int KP, const dou
   for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   const double nb = __shfl_down_sync(0xffffffffu, a, parts);
   if (part == 0 && (j & 1) == 0 && j < k)
-    ll_st2(ax + (size_t)(j >> 1) * Gs * 2, ll_wordf((float)a, seq), ll_wordf(j + 1 < k ? (float)nb : 0.f, seq));
-}
-
-// Polite wait (many CTAs poll the same words: pause between polls so that the producers' stores are not queued behind them).
-__device__ __forceinline__ void ll_wait2_polite(const u64* p, unsigned seq, u64& a, u64& b, unsigned* status) {
-  unsigned spins = 0;
-  ll_ld2(p, a, b);
-  while ((unsigned)(a >> 32) != seq || (unsigned)(b >> 32) != seq) {
-    __nanosleep(64);
-    ll_ld2(p, a, b);
-    if (++spins > kSpinLimit) { *status = 1u; break; }
-  }
+    gl_st2(ax + (size_t)(j >> 1) * Gs * 2, ll_wordf((float)a, seq), ll_wordf(j + 1 < k ? (float)nb : 0.f, seq));
 }
 
 // ------------------------------------------------------------------------------------ the kernel
@@ -468,7 +485,6 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
   double* scr = reinterpret_cast<double*>(smem + prm.off_scr);    // kThreads
   double* ctl_s = scr + kThreads - 8;                             // [0] lambda' [1] decision (owners' test); [2] 1/|p^| [3] lambda' [4] decision (gathered)
   double* praw_s = reinterpret_cast<double*>(smem + prm.off_praw);// Ns: p~ / p^ slice of this owner
-  float* bred = reinterpret_cast<float*>(smem + prm.off_bred);    // kThreads
   float* Vb = reinterpret_cast<float*>(smem + prm.off_vb);        // NG*RPT x Kpad: unit score rows of this CTA
   float* Pc = reinterpret_cast<float*>(smem + prm.off_pc);        // Ns x Kpad: P[slice, :]   (owners)
   float* Wc = reinterpret_cast<float*>(smem + prm.off_wc);        // Ns x Kpad: W[slice, :] = (R^T V)[slice, :]
@@ -478,6 +494,14 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
   const int b = blockIdx.x;
   const long long M = prm.M;
   const int N = prm.N, K = prm.K, G = prm.G, ldr = prm.ldr, Kpad = prm.Kpad, Ns = prm.Ns, Gs = prm.Gs;
+  u64 *Qx = prm.Qx, *SBx = prm.SBx, *Bx = prm.Bx, *Ax = prm.Ax, *Px = prm.Px, *Nx = prm.Nx;
+  if (prm.off_x >= 0) {                                            // one CTA: exchange through shared memory
+    u64* xb = reinterpret_cast<u64*>(smem + prm.off_x);
+    Qx = xb; SBx = Qx + 2 * (size_t)ldr; Bx = SBx + 4 * (1 + (Kpad >> 1)); Ax = Bx + 4 * (2 + Kpad); Px = Ax + 4 * (Kpad >> 1);
+    Nx = Px + 2 * (size_t)ldr;
+    const int nw = (int)(Nx + 2 * (Gs * 2 + 4) - xb);
+    for (int i = tid; i < nw; i += kThreads) xb[i] = 0ULL;         // sequence numbers start at 0
+  }
   double* pt_s = praw_s + Ns;                                      // Ns: R^T t slice (p~ before the loads-side projection), for W
   const int UB = 1 + (Kpad >> 1), UA = Kpad >> 1;                  // 2-word units per parity buffer of SBx / Ax
   const int KV = Kpad | 1;                                         // odd row stride of the shared-memory panels Vb, Pc, Wc
@@ -517,8 +541,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
     ++seq;
     {
       const unsigned par = seq & 1u;
-      reg_publish_q<GT>(prm, qs, prm.Qx + (size_t)par * Gs * G * Ns, b, seq);
-      reg_publish_sb(Vb, KV, ttil_s, sgrp, prm.SBx + ((size_t)par * UB * G + b) * 2, G, NG, mb, k, false, seq);
+      reg_publish_q<GT>(prm, qs, Qx + (size_t)par * Gs * G * Ns, b, seq);
+      reg_publish_sb(Vb, KV, ttil_s, sgrp, SBx + ((size_t)par * UB * G + b) * 2, G, NG, mb, k, false, seq);
     }
     reg_trace(prm, tn, TR_LOADS_DONE);
 
@@ -535,25 +559,25 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         // level 1: the 2-word units of [ |t~|^2 | B ] are dealt out to the duty CTAs (the non-owners if there are enough)
         const int duty0 = (G - Gs >= 16) ? Gs : 0, nduty = G - duty0;
         if (b >= duty0) {
-          const u64* sbase = prm.SBx + (size_t)par * UB * G * 2;
+          const u64* sbase = SBx + (size_t)par * UB * G * 2;
           for (int u = (b - duty0) + w * nduty; u < U; u += kWarps * nduty) {
             double a0, a1;
             reg_ll_unit<5>(sbase + (size_t)u * G * 2, 2, G, 0, u == 0, seq, status, a0, a1);
             if (lane == 0) {
-              u64* bx = prm.Bx + ((size_t)par * (2 + Kpad) + 2 * u) * 2;
-              ll_st2d(bx, a0, seq);
-              ll_st2d(bx + 2, a1, seq);
+              u64* bx = Bx + ((size_t)par * (2 + Kpad) + 2 * u) * 2;
+              gl_st2d(bx, a0, seq);
+              gl_st2d(bx + 2, a1, seq);
             }
           }
         }
       }
       if (owner) {
         RegGather gq;
-        gq.base = prm.Qx + ((size_t)par * Gs + b) * G * Ns; gq.stride = Ns; gq.hp = min(Ns >> 1, kThreads); gq.npairs = Ns >> 1;
+        gq.base = Qx + ((size_t)par * Gs + b) * G * Ns; gq.stride = Ns; gq.hp = min(Ns >> 1, kThreads); gq.npairs = Ns >> 1;
         gq.nparts = G; gq.f64_pair0 = false; gq.red = reinterpret_cast<double2*>(qs); gq.out = praw_s;
         // [ |t~|^2 | B ] summed directly: warp u takes unit u (<= 16 units, plan: kdirect <= 30), lanes over the parts (contiguous)
         const int usb = two_now ? 0 : (1 + (with_b ? ((k + 1) >> 1) : 0));
-        const u64* ub = prm.SBx + ((size_t)par * UB + w) * G * 2;
+        const u64* ub = SBx + ((size_t)par * UB + w) * G * 2;
         u64 sx[5], sy[5];
         const bool sbw = w < usb && (w > 0 || b == 0);                       // |t~|^2 (unit 0) is read by owner 0 only: it alone tests
         if (sbw) {
@@ -561,7 +585,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           for (int i2 = 0; i2 < 5; ++i2) {
             const int part = lane + 32 * i2;
             sx[i2] = 0; sy[i2] = 0;
-            if (part < G) ll_ld2(ub + (size_t)part * 2, sx[i2], sy[i2]);
+            if (part < G) gl_ld2(ub + (size_t)part * 2, sx[i2], sy[i2]);
           }
         }
         __syncthreads();                                                      // qs (group partials of the sweep) is free
@@ -574,7 +598,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
             double a0 = 0.0, a1 = 0.0;
             for (int part = 0; part < G; ++part) {
               u64 xx = 0, yy = 0;
-              ll_wait2(gq.base + (size_t)part * Ns + 2 * pr2, seq, xx, yy, status);
+              gl_wait2(gq.base + (size_t)part * Ns + 2 * pr2, seq, xx, yy, status);
               a0 += (double)ll_f(xx); a1 += (double)ll_f(yy);
             }
             praw_s[2 * pr2] = a0; praw_s[2 * pr2 + 1] = a1;
@@ -586,14 +610,14 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           for (int i2 = 0; i2 < 5; ++i2) {
             const int part = lane + 32 * i2;
             if (part < G) {
-              ll_wait2(ub + (size_t)part * 2, seq, sx[i2], sy[i2], status);
+              gl_wait2(ub + (size_t)part * 2, seq, sx[i2], sy[i2], status);
               if (w == 0) a0 += ll_d(sx[i2], sy[i2]);
               else { a0 += (double)ll_f(sx[i2]); a1 += (double)ll_f(sy[i2]); }
             }
           }
           for (int part = lane + 160; part < G; part += 32) {
             u64 xx = 0, yy = 0;
-            ll_wait2(ub + (size_t)part * 2, seq, xx, yy, status);
+            gl_wait2(ub + (size_t)part * 2, seq, xx, yy, status);
             if (w == 0) a0 += ll_d(xx, yy);
             else { a0 += (double)ll_f(xx); a1 += (double)ll_f(yy); }
           }
@@ -606,10 +630,10 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           reg_gather_store(gq);
         }
         if (two_now) {                                                        // hop 1b: gather |t~|^2 and B
-          const u64* bx = prm.Bx + (size_t)par * (2 + Kpad) * 2;
+          const u64* bx = Bx + (size_t)par * (2 + Kpad) * 2;
           for (int e = tid; e < 2 * U; e += kThreads) {
             u64 x = 0, y = 0;
-            ll_wait2(bx + 2 * e, seq, x, y, status);
+            gl_wait2(bx + 2 * e, seq, x, y, status);
             sb_s[e] = ll_d(x, y);
           }
         }
@@ -644,12 +668,12 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         // S3: a_S[j] = sum_{n in S} P[n,j] p~[n]
         if (gs)
           for (int i2 = tid; i2 < Ns; i2 += kThreads) pt_s[i2] = praw_s[i2];
-        if (gsk) reg_publish_a(Pc, KV, praw_s, prm.Ax + ((size_t)par * UA * Gs + b) * 2, Gs, ns, k, seq);
+        if (gsk) reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * UA * Gs + b) * 2, Gs, ns, k, seq);
         const int st = reinterpret_cast<const int*>(ctl_s + 1)[0];
         reg_trace(prm, tn, TR_TEST);
         if (gsk) {                                                            // (also on the pass that reports "done": only owner 0 knows)
           // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
-          reg_ll_reduce_all(prm.Ax + (size_t)par * UA * Gs * 2, 2, Gs * 2, Gs, (k + 1) >> 1, seq, status, A_s);
+          reg_ll_reduce_all(Ax + (size_t)par * UA * Gs * 2, 2, Gs * 2, Gs, (k + 1) >> 1, seq, status, A_s);
           __syncthreads();
           reg_trace(prm, tn, TR_X2);
           reg_slice_correct(praw_s, Pc, KV, A_s, ns, k);
@@ -661,16 +685,16 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           for (int u = lane; 2 * u < Ns; u += 32) {
             const float v0 = (2 * u < ns) ? (float)praw_s[2 * u] : 0.f;
             const float v1 = (2 * u + 1 < ns) ? (float)praw_s[2 * u + 1] : 0.f;
-            ll_st2(prm.Px + (size_t)par * ldr + n0 + 2 * u, ll_wordf(v0, seq), ll_wordf(v1, seq));
+            gl_st2(Px + (size_t)par * ldr + n0 + 2 * u, ll_wordf(v0, seq), ll_wordf(v1, seq));
             q2 += (double)v0 * (double)v0 + (double)v1 * (double)v1;
           }
           q2 = warp_sum(q2);
           if (lane == 0) {
-            u64* nx = prm.Nx + (size_t)par * (Gs * 2 + 4);
-            ll_st2d(nx + (size_t)b * 2, q2, seq);
+            u64* nx = Nx + (size_t)par * (Gs * 2 + 4);
+            gl_st2d(nx + (size_t)b * 2, q2, seq);
             if (b == 0) {                                                     // every owner takes the same decision: owner 0 reports it
-              ll_st2(nx + (size_t)Gs * 2, ll_word((unsigned)st, seq), ll_word(0u, seq));
-              ll_st2d(nx + (size_t)Gs * 2 + 2, ctl_s[0], seq);
+              gl_st2(nx + (size_t)Gs * 2, ll_word((unsigned)st, seq), ll_word(0u, seq));
+              gl_st2d(nx + (size_t)Gs * 2 + 2, ctl_s[0], seq);
             }
           }
         }
@@ -680,26 +704,26 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       // barrier; only then does every thread load its words of p^ (each validated by its own sequence number, so the hint
       // orders nothing).  Measured: with all 148 x 512 threads polling the same 8 KB the hop takes 2.9-3.3 us, this way 1.8 us.
       if (tid == (kWarps - 1) * 32) {
-        const u64* nxl = prm.Nx + (size_t)par * (Gs * 2 + 4) + (size_t)(Gs - 1) * 2;
+        const u64* nxl = Nx + (size_t)par * (Gs * 2 + 4) + (size_t)(Gs - 1) * 2;
         u64 x = 0, y = 0;
-        ll_wait2(nxl, seq, x, y, status);
+        gl_wait2(nxl, seq, x, y, status);
       }
       __syncthreads();
       // ---- hop 3 (every CTA): gather p^, |p^|^2, the decision and lambda' ----
       if (w == kWarps - 1) {
-        const u64* nx = prm.Nx + (size_t)par * (Gs * 2 + 4);
+        const u64* nx = Nx + (size_t)par * (Gs * 2 + 4);
         double nsum = 0.0, lamv = 0.0;
         unsigned stv = 0;
         u64 x1 = 0, y1 = 0, x2 = 0, y2 = 0;
-        if (lane == 0) { ll_ld2(nx + (size_t)Gs * 2, x1, y1); ll_ld2(nx + (size_t)Gs * 2 + 2, x2, y2); }
+        if (lane == 0) { gl_ld2(nx + (size_t)Gs * 2, x1, y1); gl_ld2(nx + (size_t)Gs * 2 + 2, x2, y2); }
         for (int o = lane; o < Gs; o += 32) {
           u64 x0 = 0, y0 = 0;
-          ll_wait2(nx + (size_t)o * 2, seq, x0, y0, status);
+          gl_wait2(nx + (size_t)o * 2, seq, x0, y0, status);
           nsum += ll_d(x0, y0);
         }
         if (lane == 0) {
-          ll_wait2(nx + (size_t)Gs * 2, seq, x1, y1, status);
-          ll_wait2(nx + (size_t)Gs * 2 + 2, seq, x2, y2, status);
+          gl_wait2(nx + (size_t)Gs * 2, seq, x1, y1, status);
+          gl_wait2(nx + (size_t)Gs * 2 + 2, seq, x2, y2, status);
           stv = (unsigned)x1;
           lamv = ll_d(x2, y2);
         }
@@ -711,7 +735,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         }
       }
       {
-        const u64* px = prm.Px + (size_t)par * ldr;
+        const u64* px = Px + (size_t)par * ldr;
         float* pg = p_s + (size_t)(it & 1) * ldr;
         for (int u0 = tid; 2 * u0 < ldr; u0 += kThreads * 4) {
           u64 x[4], y[4];
@@ -719,13 +743,13 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           for (int i = 0; i < 4; ++i) {
             const int u = u0 + i * kThreads;
             x[i] = 0; y[i] = 0;
-            if (2 * u < ldr) ll_ld2(px + 2 * u, x[i], y[i]);
+            if (2 * u < ldr) gl_ld2(px + 2 * u, x[i], y[i]);
           }
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int u = u0 + i * kThreads;
             if (2 * u < ldr) {
-              ll_wait2(px + 2 * u, seq, x[i], y[i], status);
+              gl_wait2(px + 2 * u, seq, x[i], y[i], status);
               *reinterpret_cast<float2*>(pg + 2 * u) = make_float2(ll_f(x[i]), ll_f(y[i]));
             }
           }
@@ -750,8 +774,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         const unsigned npar = seq & 1u;
         reg_sweep_fused<GT, NV, RPT>(Rr, p_s + (size_t)((it - 1) & 1) * ldr, pscale, ttil_s, qs, red_s, sgrp, ldr);
         reg_trace(prm, tn, TR_SWEEP);
-        reg_publish_q<GT>(prm, qs, prm.Qx + (size_t)npar * Gs * G * Ns, b, seq);
-        reg_publish_sb(Vb, KV, ttil_s, sgrp, prm.SBx + ((size_t)npar * UB * G + b) * 2, G, NG, mb, k, gsk, seq);
+        reg_publish_q<GT>(prm, qs, Qx + (size_t)npar * Gs * G * Ns, b, seq);
+        reg_publish_sb(Vb, KV, ttil_s, sgrp, SBx + ((size_t)npar * UB * G + b) * 2, G, NG, mb, k, gsk, seq);
         reg_trace(prm, tn, TR_PUBLISHED);
       }
     }
@@ -774,14 +798,14 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       const unsigned par = seq & 1u;
       if (gsk && !owner) {                                                    // everybody needs B for t = t~ - V B
         if (two) {
-          const u64* bx = prm.Bx + (size_t)par * (2 + Kpad) * 2;
+          const u64* bx = Bx + (size_t)par * (2 + Kpad) * 2;
           for (int e = tid; e < 2 * U; e += kThreads) {
             u64 x = 0, y = 0;
-            ll_wait2(bx + 2 * e, seq, x, y, status);
+            gl_wait2(bx + 2 * e, seq, x, y, status);
             sb_s[e] = ll_d(x, y);
           }
         } else {
-          reg_ll_reduce_all(prm.SBx + ((size_t)par * UB + 1) * G * 2, 2, G * 2, G, (k + 1) >> 1, seq, status, B_s);
+          reg_ll_reduce_all(SBx + ((size_t)par * UB + 1) * G * 2, 2, G * 2, G, (k + 1) >> 1, seq, status, B_s);
         }
         __syncthreads();
       }

@@ -198,6 +198,8 @@ def roofline(prob, run_ms_mean, peaks):
                    else "pca_solve_kernel") + " (persistent; all passes of all components in one launch)",
         "achieved": round(achieved, 1), "peak": peak, "peak_source": peaks["source"], "unit": "GB/s",
         "frac": round(achieved / peak, 4), "traffic": peaks.get("traffic"),
+        "traffic_note": "not captured for this launch (full solve); profiles/ r01b: dram read+write = 0.89 x the single-sweep "
+                        "algorithmic bytes for the same kernel on a fixed-work launch of config 4" if single else None,
         "algorithmic_bytes_per_launch": int(nbytes), "inner_iterations_per_launch": total_iters,
         "us_per_inner_iteration": round(run_ms_mean * 1e3 / max(total_iters, 1), 3),
         "bytes_model": ("single-sweep (SURVEY 8(f) F1): 4MN + [GS]4k(M+N) + 8(M+N) per inner iteration, + 4MN (R^T t0 sweep) "

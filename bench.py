@@ -424,6 +424,53 @@ def run_reference_arm(args):
     print(json.dumps(out), flush=True)
 
 
+# ------------------------------------------------------------------------------------------------
+# Fig.-1-shaped sweep: the paper's own workload: seeded
+# uniform [0,1) X, N = M/2, K = 10, eps = 1e-7, both algorithms.  Reports the GS-PCA overhead over
+# NIPALS-PCA (paper: "only about 5-7 % slower") and the per-pass speed-up over the CPU oracle next to the
+# paper's "about 12 times" (GTX280 vs one Phenom core, double precision; context, not a target).
+# ------------------------------------------------------------------------------------------------
+def run_fig1(args):
+    import torch
+    import oracle
+    from paper_0811_1081_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --fig1: no CUDA device -- the library has no CPU fallback")
+    torch.cuda.set_device(0)
+    sizes = [int(x) for x in args.fig1_sizes.split(",")]
+    rows = []
+    for i, M in enumerate(sizes):
+        N, K = M // 2, 10
+        cfg = inputs.Config(f"fig1_{M}x{N}", M, N, K, 1e-7, 10000, (inputs.ALGO_GS, inputs.ALGO_NIPALS), "uniform",
+                            seed=inputs.BASE_SEED + 100 + i, note="paper workload: uniform [0,1), N = M/2, K = 10")
+        pr = inputs.generate(cfg)
+        row = {"M": M, "N": N, "K": K}
+        for algo, tag in ((inputs.ALGO_NIPALS, "nipals"), (inputs.ALGO_GS, "gs")):
+            prob = GpuProblem(cfg, algo, pr.X)
+            step_ms, run_ms = time_steps(prob, 3, 2)
+            its = prob.iters.cpu().numpy()
+            row[tag] = {"ms_per_solve": round(float(np.mean(step_ms)), 3), "inner_iterations": int(its.sum()),
+                        "hit_max_iter": int((its >= cfg.max_iter).sum()), "plan": prob.ctx.info()["path"],
+                        "us_per_inner_iteration": round(float(np.mean(run_ms)) * 1e3 / max(int(its.sum()), 1), 3)}
+            # oracle: per-pass time on a bounded sample (eps = 0: exactly J passes of the first component)
+            Xc = oracle.center(pr.X)
+            J = max(2, min(50, int(2e8 / (M * N))))
+            t0 = time.perf_counter()
+            oracle.pca(Xc, 1, 0.0, J, algo, want_residual=False)
+            row[tag]["oracle_us_per_inner_iteration"] = round((time.perf_counter() - t0) / J * 1e6, 1)
+            row[tag]["speedup_per_pass_vs_oracle"] = round(row[tag]["oracle_us_per_inner_iteration"] /
+                                                           row[tag]["us_per_inner_iteration"], 1)
+            del prob
+            torch.cuda.empty_cache()
+        row["gs_over_nipals_time"] = round(row["gs"]["ms_per_solve"] / row["nipals"]["ms_per_solve"], 4)
+        row["gs_over_nipals_per_pass"] = round(row["gs"]["us_per_inner_iteration"] / row["nipals"]["us_per_inner_iteration"], 4)
+        rows.append(row)
+    print(json.dumps({"fig1": rows, "oracle_cores": oracle.num_threads(), "dtype": "f32 (oracle f64)", "data": "synthetic",
+                      "paper": {"speedup": "about 12x at M = 1.5e4 (GTX280 vs Phenom 9950 one core, fp64, whole solve incl. "
+                                           "transfers; PAPER.md:188)", "gs_over_nipals": "5-7 % slower (PAPER.md:188)"}}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -438,7 +485,11 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fig1", action="store_true", help="Fig.-1-shaped sweep (paper's workload) instead of the contract line")
+    ap.add_argument("--fig1-sizes", default="512,1024,2048,4096,8192,15000")
     args = ap.parse_args()
+    if args.fig1:
+        return run_fig1(args)
     world = int(os.environ.get("WORLD_SIZE", 1))
     if args.gpus != world and args.impl == "cuda":
         if world == 1 and args.gpus > 1:

@@ -130,6 +130,24 @@ def test_small_parity(binding, oracle_mod, ci, M, N, K, path, ctas, algo):
         assert mask.all(), "configs 1 and 2 have a separated spectrum by construction"
 
 
+@pytest.mark.parametrize("algo", [inputs.ALGO_GS, inputs.ALGO_NIPALS])
+def test_paper_workload_uniform(binding, oracle_mod, algo):
+    """the paper's own workload (uniform [0,1) X, N = M/2, K = 10) at a size
+    the oracle finishes in seconds.  The bulk of a centred uniform matrix is unseparated, so what is compared is what is
+    unique: the separated components one by one, and for all of them orthogonality, eq. (4), the energy identity and
+    the captured energy sum(lambda^2) against the oracle's."""
+    cfg = inputs.Config("fig1_1024x512", 1024, 512, 10, 1e-7, 10000, (algo,), "uniform", seed=inputs.BASE_SEED + 100)
+    pr = inputs.generate(cfg)
+    Xc, ref = _oracle_run(oracle_mod, pr.X, cfg, algo)
+    got = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, algo, center=True, want_residual=True)
+    what = f"{cfg.name} algo={algo} {got['info']['path']}"
+    mask = separated_mask(ref.lam, cfg.K)
+    assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
+    _check_invariants(got, f64(got["Xc"]), algo, cfg.K, what)
+    e_g, e_o = float(np.sum(f64(got["lam"]) ** 2)), float(np.sum(ref.lam[:cfg.K] ** 2))
+    assert abs(e_g - e_o) <= 1e-3 * e_o, f"{what} captured energy {e_g} vs {e_o}"
+
+
 def test_paths_agree_and_are_deterministic(binding):
     """Resident and streaming plans run the same arithmetic in the same order per CTA count;
     each plan is bitwise reproducible run to run (fixed-order reductions)."""

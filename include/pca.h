@@ -106,7 +106,8 @@ enum {
  *   K         number of components, 1 <= K <= N ("K <= N"; the start vector of
  *             component k is column k of the residual)
  *   eps       >= 0; relative stagnation tolerance of the listings' test
- *             |lambda - lambda'| < eps * lambda'.  eps = 0 never fires,
+ *             |lambda - lambda'| < eps * lambda'; lambda' is also compared with
+ *             the value two passes back (a period-2 limit cycle in fp32 is stagnation, C4b).  eps = 0 never fires,
  *             i.e. exactly max_iter passes per component (fixed-work benchmark mode)
  *   max_iter  >= 1; the listings' J = 10000
  *   algo      PCA_ALGO_NIPALS or PCA_ALGO_GS

@@ -489,7 +489,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
     }
     trace_mark(prm, tn, TR_LOADS_DONE);
 
-    double lam = 0.0, lam_new = 0.0;
+    double lam = 0.0, lam2 = 0.0, lam_new = 0.0;
     int it = 0;
     bool degenerate = false;
     bool first = true;
@@ -527,7 +527,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           else {
             ln = sqrt(l2);                                                    // S7
             // S8: listings' strict relative test (reading C3)
-            if ((fabs(lam - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
+            // (+ reading C4b: a period-2 limit cycle of lambda' in fp32 is stagnation too)
+            if ((fabs(lam - ln) < prm.eps * ln) || (fabs(lam2 - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
           }
         }
         if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }
@@ -557,7 +558,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       if (!first) {
         lam_new = ctl_s[0];
         done = st == 1;
-        if (!done) lam = lam_new;
+        if (!done) { lam2 = lam; lam = lam_new; }
       }
       trace_mark(prm, tn, TR_TEST);
       if (done) break;

@@ -49,7 +49,8 @@ struct RegParams {
   unsigned long long* SBx;  // [2][1 + Kpad/2][G][2] UNIT-major (a warp polling one unit over the parts reads contiguous
                             //                     words): unit 0 = partial |t~|^2 (fp64 bits), unit 1+j/2 = partial (B[j], B[j+1]) (fp32)
   unsigned long long* Bx;   // [2][2 + Kpad][2]    two-level: entry e as fp64 bits (entry 0 = |t~|^2, entry 2+j = B[j])
-  unsigned long long* Ax;   // [2][Kpad/2][Gs][2]  partial (A[j], A[j+1]) (fp32), unit-major
+  unsigned long long* Ax;   // [2][Gs*Kpad]        partial A (fp32) of each owner; k <= 64: unit-major [Kpad/2][Gs][2] (a warp per unit,
+                            //                     lanes over the owners), else owner-major [Gs][Kpad] (lanes over the units, owners in turn)
   unsigned long long* Px;   // [2][ldr]            p^ (orthogonalised, not normalised)
   unsigned long long* Nx;   // [2][Gs*2 + 4]       per owner: partial |p^|^2 (fp64, 2 words); then {decision, -, lambda' (fp64)}
   unsigned* status;         // [0] != 0: an exchange wait gave up
@@ -360,11 +361,22 @@ __device__ __forceinline__ void reg_gather_finish(const RegGather& gq, u64 (&x)[
         else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
       }
     }
-    for (int part = pslot + INF * pstep; part < gq.nparts; part += pstep) {   // more parts than INF rounds cover (rare)
-      u64 xx = 0, yy = 0;
-      gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, xx, yy, status);
-      if (f64) a0 += ll_d(xx, yy);
-      else { a0 += (double)ll_f(xx); a1 += (double)ll_f(yy); }
+    for (int p0 = pslot + INF * pstep; p0 < gq.nparts; p0 += INF * pstep) {     // more parts than one batch covers
+#pragma unroll
+      for (int i = 0; i < INF; ++i) {
+        const int part = p0 + i * pstep;
+        x[i] = 0; y[i] = 0;
+        if (part < gq.nparts) gl_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
+      }
+#pragma unroll
+      for (int i = 0; i < INF; ++i) {
+        const int part = p0 + i * pstep;
+        if (part < gq.nparts) {
+          gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
+          if (f64) a0 += ll_d(x[i], y[i]);
+          else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
+        }
+      }
     }
   }
   for (int o = 16; o >= hp; o >>= 1) {                                        // lanes l and l ^ o own the same pair when o >= hp
@@ -426,7 +438,18 @@ __device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const fl
   const int j = tid / parts, part = tid - j * parts;
   float a = 0.f;
   if (j < k)
-    for (int r = part; r < mb; r += parts) a = fmaf(Vb[(size_t)r * KV + j], ttil_s[r], a);
+  {
+    float a1 = 0.f, a2 = 0.f, a3 = 0.f;                                  // four independent chains (fixed association)
+    int r = part;
+    for (; r + 3 * parts < mb; r += 4 * parts) {                       // (no trip when a thread has fewer than 4 rows)
+      a = fmaf(Vb[(size_t)r * KV + j], ttil_s[r], a);
+      a1 = fmaf(Vb[(size_t)(r + parts) * KV + j], ttil_s[r + parts], a1);
+      a2 = fmaf(Vb[(size_t)(r + 2 * parts) * KV + j], ttil_s[r + 2 * parts], a2);
+      a3 = fmaf(Vb[(size_t)(r + 3 * parts) * KV + j], ttil_s[r + 3 * parts], a3);
+    }
+    for (; r < mb; r += parts) a = fmaf(Vb[(size_t)r * KV + j], ttil_s[r], a);
+    a = (a + a1) + (a2 + a3);
+  }
   for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   const float nb = __shfl_down_sync(0xffffffffu, a, parts);             // column j + 1 (same part)
   if (part == 0 && (j & 1) == 0 && j < k)
@@ -451,8 +474,8 @@ __device__ __forceinline__ void reg_slice_correct(double* praw_s, const float* C
 }
 
 // S3, first half: this owner's partial  a_S[j] = sum_{n in S} P[n,j] p~[n], all threads of the CTA.
-__device__ __forceinline__ void reg_publish_a(const float* Pc, int KP, const double* praw_s, u64* ax, int Gs, int ns, int k,
-                                              unsigned seq) {   // ax: this owner's slot of unit 0
+__device__ __forceinline__ void reg_publish_a(const float* Pc, int KP, const double* praw_s, u64* ax, int ustride, int ns, int k,
+                                              unsigned seq) {   // ax: this owner's slot of unit 0; ustride: words between units
   const int tid = threadIdx.x;
   int Kc = 32;
   while (Kc < k) Kc <<= 1;
@@ -464,7 +487,7 @@ __device__ __forceinline__ void reg_publish_a(const float* Pc, int KP, const dou
   for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   const double nb = __shfl_down_sync(0xffffffffu, a, parts);
   if (part == 0 && (j & 1) == 0 && j < k)
-    gl_st2(ax + (size_t)(j >> 1) * Gs * 2, ll_wordf((float)a, seq), ll_wordf(j + 1 < k ? (float)nb : 0.f, seq));
+    gl_st2(ax + (size_t)(j >> 1) * ustride, ll_wordf((float)a, seq), ll_wordf(j + 1 < k ? (float)nb : 0.f, seq));
 }
 
 // ------------------------------------------------------------------------------------ the kernel
@@ -503,7 +526,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
     for (int i = tid; i < nw; i += kThreads) xb[i] = 0ULL;         // sequence numbers start at 0
   }
   double* pt_s = praw_s + Ns;                                      // Ns: R^T t slice (p~ before the loads-side projection), for W
-  const int UB = 1 + (Kpad >> 1), UA = Kpad >> 1;                  // 2-word units per parity buffer of SBx / Ax
+  const int UB = 1 + (Kpad >> 1);                                  // 2-word units per parity buffer of SBx
   const int KV = Kpad | 1;                                         // odd row stride of the shared-memory panels Vb, Pc, Wc
   const bool gs = prm.algo == 1;
   const long long m0 = (long long)b * prm.Mb;
@@ -546,7 +569,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
     }
     reg_trace(prm, tn, TR_LOADS_DONE);
 
-    double lam = 0.0, lam_new = 0.0;
+    double lam = 0.0, lam2 = 0.0, lam_new = 0.0;                    // lambda of the previous pass, of the one before, of this one
     int it = 0;
     bool degenerate = false, first = true;
     float pscale = 0.f;
@@ -658,7 +681,9 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
             else {
               ln = sqrt(l2);                                                  // S7
               // S8: the listings' strict relative test (reading C3)
-              if ((fabs(lam - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
+              // (+ reading C4b: in fp32 the iteration can end in a period-2 limit cycle, lambda' alternating between two
+              //  values; that is stagnation too, so lambda' is also compared with the value two passes back)
+              if ((fabs(lam - ln) < prm.eps * ln) || (fabs(lam2 - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
             }
           }
           if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }
@@ -668,12 +693,29 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         // S3: a_S[j] = sum_{n in S} P[n,j] p~[n]
         if (gs)
           for (int i2 = tid; i2 < Ns; i2 += kThreads) pt_s[i2] = praw_s[i2];
-        if (gsk) reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * UA * Gs + b) * 2, Gs, ns, k, seq);
+        if (gsk) {
+          if (k <= 64) reg_publish_a(Pc, KV, praw_s, Ax + (size_t)par * Gs * Kpad + (size_t)b * 2, Gs * 2, ns, k, seq);
+          else reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * Gs + b) * Kpad, 2, ns, k, seq);
+        }
         const int st = reinterpret_cast<const int*>(ctl_s + 1)[0];
         reg_trace(prm, tn, TR_TEST);
         if (gsk) {                                                            // (also on the pass that reports "done": only owner 0 knows)
           // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
-          reg_ll_reduce_all(Ax + (size_t)par * UA * Gs * 2, 2, Gs * 2, Gs, (k + 1) >> 1, seq, status, A_s);
+          if (k <= 64) {                                                      // few units: a warp per unit, lanes over the owners
+            reg_ll_reduce_all(Ax + (size_t)par * Gs * Kpad, 2, Gs * 2, Gs, (k + 1) >> 1, seq, status, A_s);
+          } else {                                                            // many units: lanes over the units (coalesced), owners in turn
+            RegGather ga;
+            const int ua = (k + 1) >> 1;
+            int ha = 1;
+            while (ha < ua) ha <<= 1;
+            ga.base = Ax + (size_t)par * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
+            ga.f64_pair0 = false; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
+            u64 ax8[8], ay8[8];
+            reg_gather_issue<8>(ga, ax8, ay8);
+            reg_gather_finish<8>(ga, ax8, ay8, seq, status);
+            __syncthreads();
+            reg_gather_store(ga);
+          }
           __syncthreads();
           reg_trace(prm, tn, TR_X2);
           reg_slice_correct(praw_s, Pc, KV, A_s, ns, k);
@@ -762,6 +804,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       if (!first) {
         lam_new = ctl_s[3];
         if (st3 == 1) break;
+        lam2 = lam;
         lam = lam_new;
       }
       pscale = reinterpret_cast<const float*>(ctl_s + 2)[0];                   // p = p^/|p^|

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
     }
     __syncthreads();
 
-    double lam = 0.0, lam_new = 0.0;
+    double lam = 0.0, lam2 = 0.0, lam_new = 0.0;
     int it = 0;
     bool degenerate = false;
     for (int j = 0; j < prm.max_iter; ++j) {
@@ -224,7 +224,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       }
       it = j + 1;
       // ---- S8: listings' strict relative test (reading C3) ----
-      if (fabs(lam - lam_new) < prm.eps * lam_new) break;
+      if (fabs(lam - lam_new) < prm.eps * lam_new || fabs(lam2 - lam_new) < prm.eps * lam_new) break;   // (reading C4b)
+      lam2 = lam;
       lam = lam_new;
     }
 

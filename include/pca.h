@@ -57,7 +57,8 @@ enum {
 enum {
   PCA_OPT_PATH = 1,     /* 0 = auto; two-sweep kernel: 1 = HBM-streaming, 2 = SMEM-resident;
                            single-sweep kernel (R read once per inner pass): 3 = streaming, 4 = SMEM-resident,
-                           5 = register-resident (4*M*N up to ~19 MB on 148 SMs) */
+                           5 = register-resident (4*M*N up to ~19 MB on 148 SMs), 6 = one CTA (the matrix in the registers
+                           of one SM: N <= 512, M <= (512/GT)*7 rows with GT = pow2 >= N/8) */
   PCA_OPT_CTAS = 2,     /* number of CTAs of the persistent kernel (0 = auto) */
   PCA_OPT_CENTER_MODE = 3, /* 0 = column means (default), 1 = literal eq. (1) mean column */
   PCA_OPT_OWNERS = 5,   /* register-resident kernel: number of slice-owner CTAs (0 = auto; rounded down to a power of two) */
@@ -88,7 +89,7 @@ enum {
 /* Fields for pca_get_info. */
 enum {
   PCA_INFO_PATH = 1,        /* 1, 2 = two-sweep kernel streaming / resident; 3, 4 = single-sweep kernel streaming / resident;
-                               5 = register-resident single-sweep kernel */
+                               5 = register-resident single-sweep kernel; 6 = one-CTA single-sweep kernel */
   PCA_INFO_CTAS = 2,        /* CTAs of the persistent solve kernel */
   PCA_INFO_THREADS = 3,     /* threads per CTA */
   PCA_INFO_SMEM_BYTES = 4,  /* dynamic shared memory per CTA */

@@ -20,7 +20,7 @@ PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED = ra
 
 PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT = 1, 2, 3, 4, 5, 6
 (PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT,
- PCA_PATH_REGISTER) = 0, 1, 2, 3, 4, 5
+ PCA_PATH_REGISTER, PCA_PATH_ONE_CTA) = 0, 1, 2, 3, 4, 5, 6
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
  PCA_INFO_LAUNCHES_PER_RUN, PCA_INFO_NUM_SMS, PCA_INFO_ROW_GROUP_THREADS, PCA_INFO_RUN_STATUS, PCA_INFO_OWNERS) = range(1, 11)
 
@@ -118,7 +118,7 @@ class PcaContext:
         return {
             "path": {1: "two-sweep streaming", 2: "two-sweep resident", 3: "single-sweep streaming",
                      4: "single-sweep resident",
-                     5: "single-sweep register-resident"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
+                     5: "single-sweep register-resident", 6: "single-sweep one-CTA"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
             "ctas": self.pca_get_info(PCA_INFO_CTAS),
             "threads": self.pca_get_info(PCA_INFO_THREADS),
             "smem_bytes": self.pca_get_info(PCA_INFO_SMEM_BYTES),

@@ -14,11 +14,13 @@
 
 #include "pca_center.cuh"
 #include "pca_fused.cuh"
+#include "pca_one.cuh"
 #include "pca_reg.cuh"
 #include "pca_solve.cuh"
 
 using pca::FusedParams;
 using pca::RegParams;
+using pca::OneParams;
 using pca::SolveParams;
 
 namespace {
@@ -57,6 +59,13 @@ reg_kernel_t reg_kernel_lookup_part0(int gt, int rpt);
 reg_kernel_t reg_kernel_lookup_part1(int gt, int rpt);
 reg_kernel_t reg_kernel_lookup_part2(int gt, int rpt);
 reg_kernel_t reg_kernel_lookup_part3(int gt, int rpt);
+one_kernel_t one_kernel_lookup_part0(int gt, int rpt);
+one_kernel_t one_kernel_lookup_part1(int gt, int rpt);
+one_kernel_t one_kernel_lookup(int gt, int rpt) {
+  one_kernel_t f = one_kernel_lookup_part0(gt, rpt);
+  if (!f) f = one_kernel_lookup_part1(gt, rpt);
+  return f;
+}
 reg_kernel_t reg_kernel_lookup(int gt, int rpt) {
   reg_kernel_t f = reg_kernel_lookup_part0(gt, rpt);
   if (!f) f = reg_kernel_lookup_part1(gt, rpt);
@@ -82,6 +91,8 @@ struct pca_ctx {
                  // 5 register-resident single-sweep kernel
   pca::reg_kernel_t rfn = nullptr;
   RegParams rprm{};
+  pca::one_kernel_t ofn = nullptr;   // path 6: one-CTA kernel
+  OneParams oprm{};
   int r_gt = 0, r_rpt = 0;
   size_t ws_off_bx = 0;
   const Variant* variant = nullptr;
@@ -379,8 +390,68 @@ int make_reg_plan(pca_ctx* c) {
   return PCA_OK;
 }
 
+// One-CTA kernel (pca_one.cuh): the whole matrix in the registers of one SM.  M <= (512/GT)*7, GT = pow2 >= N/8, GT <= 64.
+int make_one_plan(pca_ctx* c) {
+  const long long M = c->M, N = c->N;
+  int GT = 8;
+  while (8LL * GT < N) GT *= 2;
+  if (GT > 64) return PCA_EUNSUPPORTED;
+  const int NG = pca::kThreads / GT, ldr = 8 * GT;
+  if (M > (long long)NG * 7 || (c->opt_ctas > 1)) return PCA_EUNSUPPORTED;
+  int RPT = 0;
+  for (int r : {2, 4, 7})
+    if ((long long)NG * r >= M) { RPT = r; break; }
+  pca::one_kernel_t fn = pca::one_kernel_lookup(GT, RPT);
+  if (!fn) return PCA_EUNSUPPORTED;
+  OneParams p{};
+  p.M = (int)M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  p.ldr = ldr; p.Kpad = (int)round_up(c->K, 4);
+  const bool gs = c->algo == PCA_ALGO_GS;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 16); return (int)o; };
+  const size_t rows = (size_t)NG * RPT, KV = (size_t)(p.Kpad | 1);
+  p.off_p = take((size_t)ldr * 4);
+  p.off_ttil = take(rows * 4);
+  p.off_d = take(rows * 4);
+  p.off_qs = take((size_t)NG * ldr * 4);
+  p.off_red = take((size_t)pca::kThreads * 4);
+  p.off_sgrp = take((size_t)NG * 8);
+  p.off_q = take((size_t)ldr * 8);
+  p.off_B = take((size_t)(2 + p.Kpad) * 8);
+  p.off_A = take((size_t)(2 + p.Kpad) * 8);
+  p.off_scr = take((size_t)pca::kThreads * 8);
+  p.off_vb = take(gs ? rows * KV * 4 : 0);
+  p.off_pp = take(gs ? (size_t)ldr * KV * 4 : 0);
+  p.off_wp = take(gs ? (size_t)ldr * KV * 4 : 0);
+  const size_t smem = off;
+  if (smem > (size_t)c->smem_optin) return PCA_EUNSUPPORTED;
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  size_t woff = 0;
+  auto wtake = [&](size_t bytes) { size_t o = woff; woff = (size_t)round_up((long long)(woff + bytes), 256); return o; };
+  wtake((size_t)M * (size_t)N * 4);                                  // residual of eq. (4), column-major (ABI layout)
+  c->ws_off_rrm = wtake((size_t)M * (size_t)ldr * 4);                // row-major copy: read once, written once
+  c->ws_off_status = wtake(256);
+  c->ws_bytes = woff;
+  c->oprm = p;
+  c->ofn = fn;
+  c->r_gt = GT; c->r_rpt = RPT;
+  c->smem_bytes = smem;
+  c->path = 6;
+  c->planned = true;
+  c->ws = nullptr;
+  c->ws_given = 0;
+  c->ran = false;
+  return PCA_OK;
+}
+
 int make_plan(pca_ctx* c) {
   c->planned = false;
+  if ((c->opt_path == 0 && c->opt_trace == 0) || c->opt_path == 6) {
+    const int rc = make_one_plan(c);
+    if (rc == PCA_OK || c->opt_path != 0) return rc;
+    if (rc == PCA_ECUDA) return rc;
+  }
   if (c->opt_path == 0 || c->opt_path == 5) {
     const int rc = make_reg_plan(c);
     if (rc == PCA_OK || c->opt_path != 0) return rc;
@@ -498,7 +569,7 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
   if (!c) return PCA_EINVAL;
   switch (option) {
     case PCA_OPT_PATH:
-      if (value < 0 || value > 5) return PCA_EINVAL;
+      if (value < 0 || value > 6) return PCA_EINVAL;
       c->opt_path = (int)value;
       break;
     case PCA_OPT_CTAS:
@@ -531,17 +602,17 @@ int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
   if (!c || !value || !c->planned) return PCA_EINVAL;
   switch (field) {
     case PCA_INFO_PATH: *value = c->path; break;
-    case PCA_INFO_CTAS: *value = c->path == 5 ? c->rprm.G : (c->path >= 3 ? c->fprm.G : c->prm.G); break;
-    case PCA_INFO_OWNERS: *value = c->path == 5 ? c->rprm.Gs : (c->path >= 3 ? c->fprm.Gs : c->prm.Gs); break;
+    case PCA_INFO_CTAS: *value = c->path == 6 ? 1 : c->path == 5 ? c->rprm.G : (c->path >= 3 ? c->fprm.G : c->prm.G); break;
+    case PCA_INFO_OWNERS: *value = c->path == 6 ? 1 : c->path == 5 ? c->rprm.Gs : (c->path >= 3 ? c->fprm.Gs : c->prm.Gs); break;
     case PCA_INFO_THREADS: *value = pca::kThreads; break;
     case PCA_INFO_SMEM_BYTES: *value = (int64_t)c->smem_bytes; break;
-    case PCA_INFO_ROWS_PER_CTA: *value = c->path == 5 ? c->rprm.Mb : (c->path >= 3 ? c->fprm.Mb : c->prm.Mb); break;
+    case PCA_INFO_ROWS_PER_CTA: *value = c->path == 6 ? c->oprm.M : c->path == 5 ? c->rprm.Mb : (c->path >= 3 ? c->fprm.Mb : c->prm.Mb); break;
     case PCA_INFO_LAUNCHES_PER_RUN: *value = c->path >= 3 ? 3 : 1; break;
-    case PCA_INFO_ROW_GROUP_THREADS: *value = c->path == 5 ? c->r_gt : (c->path >= 3 ? c->fprm.GT : 0); break;
+    case PCA_INFO_ROW_GROUP_THREADS: *value = c->path >= 5 ? c->r_gt : (c->path >= 3 ? c->fprm.GT : 0); break;
     case PCA_INFO_NUM_SMS: *value = c->num_sms; break;
     case PCA_INFO_RUN_STATUS: {
       *value = 0;
-      if (c->path >= 3 && c->ws && c->ran) {
+      if (c->path >= 3 && c->path != 6 && c->ws && c->ran) {
         unsigned st = 0;
         if (cudaMemcpy(&st, static_cast<const unsigned char*>(c->ws) + c->ws_off_status, sizeof(st),
                        cudaMemcpyDeviceToHost) != cudaSuccess) return PCA_ECUDA;
@@ -587,6 +658,21 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
   if (!c->ws || c->ws_given < c->ws_bytes) return PCA_EWORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   unsigned char* ws = static_cast<unsigned char*>(c->ws);
+  if (c->path == 6) {
+    OneParams p = c->oprm;
+    p.Rrm = reinterpret_cast<float*>(ws + c->ws_off_rrm);
+    p.T = T; p.P = P; p.lambda = lambda; p.iters = iters;
+    const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
+    pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X
+    PCA_CUDA(c, cudaGetLastError());
+    c->ofn<<<1, pca::kThreads, c->smem_bytes, st>>>(p);
+    PCA_CUDA(c, cudaGetLastError());
+    const dim3 ogrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(c->N, 32));
+    pca::pca_transpose_plain_kernel<<<ogrid, 256, 0, st>>>(p.Rrm, reinterpret_cast<float*>(ws), c->M, p.N, p.ldr);
+    PCA_CUDA(c, cudaGetLastError());
+    c->ran = true;
+    return PCA_OK;
+  }
   if (c->path == 5) {
     RegParams p = c->rprm;
     p.Rrm = reinterpret_cast<float*>(ws + c->ws_off_rrm);
@@ -673,7 +759,7 @@ int pca_residual(const pca_ctx* c, const float** R) {
 
 int pca_trace(const pca_ctx* c, const uint64_t** records, int64_t* capacity) {
   if (!c || !records || !capacity) return PCA_EINVAL;
-  if (!c->planned || c->path < 3 || c->opt_trace <= 0) return PCA_EUNSUPPORTED;
+  if (!c->planned || c->path < 3 || c->path == 6 || c->opt_trace <= 0) return PCA_EUNSUPPORTED;
   if (!c->ws || !c->ran) return PCA_EWORKSPACE;
   *records = reinterpret_cast<const uint64_t*>(static_cast<const unsigned char*>(c->ws) + c->ws_off_trace);
   *capacity = c->opt_trace;

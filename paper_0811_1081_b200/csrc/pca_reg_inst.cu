@@ -1,6 +1,6 @@
 // Instantiations of the register-resident solve kernel (pca_reg.cuh), split over several translation
 // units (-DPCA_REG_PART=0..3) so that they compile in parallel.  NV = 2 (eight columns per thread and row).
-#include "pca_reg.cuh"
+#include "pca_one.cuh"
 
 #ifndef PCA_REG_PART
 #error "compile with -DPCA_REG_PART=<0..3>"
@@ -12,14 +12,26 @@ namespace pca {
   if (gt == GT && rpt == RPT) return pca_reg_kernel<GT, 2, RPT>;
 #define PCA_RV3(GT) PCA_RV(GT, 2) PCA_RV(GT, 4) PCA_RV(GT, 7)
 
+#define PCA_OV(GT, RPT) \
+  if (gt == GT && rpt == RPT) return pca_one_kernel<GT, RPT>;
+#define PCA_OV3(GT) PCA_OV(GT, 2) PCA_OV(GT, 4) PCA_OV(GT, 7)
+
 #if PCA_REG_PART == 0
 reg_kernel_t reg_kernel_lookup_part0(int gt, int rpt) {
   PCA_RV3(8) PCA_RV3(16)
   return nullptr;
 }
+one_kernel_t one_kernel_lookup_part0(int gt, int rpt) {
+  PCA_OV3(8) PCA_OV3(16)
+  return nullptr;
+}
 #elif PCA_REG_PART == 1
 reg_kernel_t reg_kernel_lookup_part1(int gt, int rpt) {
   PCA_RV3(32) PCA_RV3(64)
+  return nullptr;
+}
+one_kernel_t one_kernel_lookup_part1(int gt, int rpt) {
+  PCA_OV3(32) PCA_OV3(64)
   return nullptr;
 }
 #elif PCA_REG_PART == 2

@@ -105,6 +105,12 @@ SMALL_CASES = [
     (4, 1024, 64, 64, 5, 0),        # K = N full decomposition, 3 CTAs
     (1, 64, 300, 4, 5, 0),          # M < N
     (1, 1024, 4096, 6, 5, 0),       # 512 threads per row (one row group per CTA)
+    # one-CTA kernel (path 6; what the auto plan picks when the matrix fits the registers of one SM)
+    (0, 256, 64, 8, 6, 0),          # BASELINE.json configs[0] in full: 8 threads per row, 4 rows per thread
+    (0, 200, 50, 16, 6, 0),         # ragged rows and columns
+    (1, 100, 200, 6, 6, 0),         # M < N, 32 threads per row
+    (4, 400, 64, 64, 6, 0),         # 7 rows per thread, K = N
+    (2, 56, 500, 10, 6, 0),         # 64 threads per row, collinear columns
 ]
 
 
@@ -168,7 +174,7 @@ def test_eps_zero_runs_exactly_max_iter(binding):
     cfg = inputs.scaled(inputs.config(0), 256, 64, K=3)
     pr = inputs.generate(cfg)
     for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
-        for path in (0, 1, 2, 3, 4, 5):
+        for path in (0, 1, 2, 3, 4, 5, 6):
             got = binding.fit(pr.X, 3, 0.0, 7, algo, path=path)
             assert got["iters"].tolist() == [7, 7, 7]
         got = binding.fit(pr.X, 3, 0.0, 1, algo)               # a single pass per component

@@ -64,6 +64,8 @@ enum {
   PCA_OPT_OWNERS = 5,   /* register-resident kernel: number of slice-owner CTAs (0 = auto; rounded down to a power of two) */
   PCA_OPT_KDIRECT = 6,  /* register-resident kernel: the Gram-Schmidt coefficients B of component k are combined in two
                            levels for k > this value (-1 = default) */
+  PCA_OPT_TEST_MODE = 7, /* convergence test: 0 = the listings' strict relative test |lambda - lambda'| < eps*lambda'
+                           (default), 1 = the text's absolute test |lambda' - lambda| <= eps */
   PCA_OPT_TRACE = 4     /* single-sweep kernels only: capacity (records) of the device-side phase trace, 0 = off
                            (default).  See pca_trace. */
 };

@@ -156,11 +156,14 @@ int oracle_center_eq1(double* X, int64_t M, int64_t N) {
 //   iters  out: K, inner passes executed (1-based); == max_iter means the test never fired
 //   R      out: M x N residual after K deflations ("return T, P, R"); may be NULL
 // returns 0, or 1 on invalid arguments.
-int oracle_pca(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo,
-               double* T, double* P, double* lambda, int32_t* iters, double* R_out) {
+//   test_mode  0: the listings' strict relative test |lambda - lambda'| < eps*lambda' (reading C3, default)
+//              1: the text's / pseudo-code's absolute test |lambda' - lambda| <= eps
+int oracle_pca_ex(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo, int test_mode,
+                  double* T, double* P, double* lambda, int32_t* iters, double* R_out) {
   if (!X || !T || !P || !lambda || !iters) return 1;
   if (M < 1 || N < 1 || K < 1 || K > N || !(eps >= 0.0) || max_iter < 1) return 1;
   if (algo != 0 && algo != 1) return 1;
+  if (test_mode != 0 && test_mode != 1) return 1;
   const bool gs = (algo == 1);
 
   std::vector<double> Rv((size_t)M * (size_t)N);
@@ -203,7 +206,8 @@ int oracle_pca(const double* X, int64_t M, int64_t N, int K, double eps, int max
       if (gs)
         for (int64_t m = 0; m < M; ++m) t[m] /= lam_new;             // V^(k) <- V^(k)/lambda_k
       it = j + 1;
-      if (std::fabs(lam - lam_new) < eps * lam_new) break;           // PAPER.md:566,:1034 (C3)
+      if (test_mode == 0 ? (std::fabs(lam - lam_new) < eps * lam_new)  // PAPER.md:566,:1034 (C3)
+                         : (std::fabs(lam_new - lam) <= eps)) break;   // PAPER.md:40,:84 (text)
       lam = lam_new;
     }
     if (degenerate) {
@@ -223,6 +227,11 @@ int oracle_pca(const double* X, int64_t M, int64_t N, int K, double eps, int max
       for (int64_t m = 0; m < M; ++m) T[id(m, k, M)] *= lambda[k];
   if (R_out) std::memcpy(R_out, R, sizeof(double) * (size_t)M * (size_t)N);
   return 0;
+}
+
+int oracle_pca(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo,
+               double* T, double* P, double* lambda, int32_t* iters, double* R_out) {
+  return oracle_pca_ex(X, M, N, K, eps, max_iter, algo, 0, T, P, lambda, iters, R_out);
 }
 
 // Cyclic Jacobi eigenvalue iteration for a real symmetric n x n matrix (textbook; Golub &

@@ -18,7 +18,7 @@ PCA_ALGO_GS = 1
 
 PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED = range(6)
 
-PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT = 1, 2, 3, 4, 5, 6
+PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT, PCA_OPT_TEST_MODE = 1, 2, 3, 4, 5, 6, 7
 (PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT,
  PCA_PATH_REGISTER, PCA_PATH_ONE_CTA) = 0, 1, 2, 3, 4, 5, 6
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
@@ -235,7 +235,7 @@ def to_colmajor(t):
 
 
 def fit(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, path=PCA_PATH_AUTO, ctas=0,
-        want_residual=False):
+        want_residual=False, test_mode=0):
     """One-call helper used by tests / smoke: numpy (M, N) float32 in -> dict of numpy results.
 
     Runs pca_center (optional) and pca_run on the GPU through the C ABI."""
@@ -246,6 +246,8 @@ def fit(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, path=P
         ctx.pca_set_option(PCA_OPT_PATH, path)
     if ctas:
         ctx.pca_set_option(PCA_OPT_CTAS, ctas)
+    if test_mode:
+        ctx.pca_set_option(PCA_OPT_TEST_MODE, test_mode)
     X = from_colmajor(X_np)
     if center:
         ctx.pca_center(X)

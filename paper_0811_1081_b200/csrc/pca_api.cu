@@ -84,7 +84,7 @@ struct pca_ctx {
   // device
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
-  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1;
+  int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -258,7 +258,7 @@ int make_fused_plan(pca_ctx* c, int want) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
   take((size_t)M * (size_t)N * 4);                                   // residual of eq. (4), column-major (ABI layout)
@@ -360,7 +360,7 @@ int make_reg_plan(pca_ctx* c) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
   p.kdirect = c->opt_kdirect >= 0 ? (c->opt_kdirect > 30 ? 30 : c->opt_kdirect) : 0;    // direct: <= 16 units, one per warp
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
@@ -404,7 +404,7 @@ int make_one_plan(pca_ctx* c) {
   pca::one_kernel_t fn = pca::one_kernel_lookup(GT, RPT);
   if (!fn) return PCA_EUNSUPPORTED;
   OneParams p{};
-  p.M = (int)M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  p.M = (int)M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
   p.ldr = ldr; p.Kpad = (int)round_up(c->K, 4);
   const bool gs = c->algo == PCA_ALGO_GS;
   size_t off = 0;
@@ -508,7 +508,7 @@ int make_plan(pca_ctx* c) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo;
+  p.M = M; p.N = N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
   // workspace layout: R first
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
@@ -587,6 +587,10 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
     case PCA_OPT_KDIRECT:
       if (value < -1 || value > (1 << 30)) return PCA_EINVAL;
       c->opt_kdirect = (int)value;
+      break;
+    case PCA_OPT_TEST_MODE:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_test_mode = (int)value;
       break;
     case PCA_OPT_TRACE:
       if (value < 0 || value > (1 << 24)) return PCA_EINVAL;

@@ -52,6 +52,7 @@ struct FusedParams {
   double eps;
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
+  int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
   int G;                 // CTAs
   int Mb;                // rows per CTA
   int ldr;               // row stride of Rrm / slab (floats) = 4*GT*NV
@@ -528,7 +529,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
             ln = sqrt(l2);                                                    // S7
             // S8: listings' strict relative test (reading C3)
             // (+ reading C4b: a period-2 limit cycle of lambda' in fp32 is stagnation too)
-            if ((fabs(lam - ln) < prm.eps * ln) || (fabs(lam2 - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
+            if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode) || (it >= prm.max_iter)) st = 1;
           }
         }
         if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }

@@ -24,6 +24,7 @@ struct OneParams {
   double eps;
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
+  int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
   int ldr;               // 8*GT >= N
   int Kpad;
   // shared-memory carve-up (byte offsets)
@@ -157,7 +158,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
           else {
             ln = sqrt(l2);                                                    // S7
             // S8: the listings' strict relative test (readings C3, C4b)
-            if ((fabs(lam - ln) < prm.eps * ln) || (fabs(lam2 - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
+            if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode) || (it >= prm.max_iter)) st = 1;
           }
         }
         if (lane == 0) { ctl_s[1] = ln; reinterpret_cast<int*>(ctl_s + 2)[0] = st; }

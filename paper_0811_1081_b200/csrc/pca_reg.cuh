@@ -38,6 +38,7 @@ struct RegParams {
   double eps;
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
+  int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
   int G;                 // CTAs
   int Mb;                // rows per CTA (<= NG*RPT)
   int ldr;               // 4*NV*GT >= N
@@ -683,7 +684,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
               // S8: the listings' strict relative test (reading C3)
               // (+ reading C4b: in fp32 the iteration can end in a period-2 limit cycle, lambda' alternating between two
               //  values; that is stagnation too, so lambda' is also compared with the value two passes back)
-              if ((fabs(lam - ln) < prm.eps * ln) || (fabs(lam2 - ln) < prm.eps * ln) || (it >= prm.max_iter)) st = 1;
+              if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode) || (it >= prm.max_iter)) st = 1;
             }
           }
           if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }

@@ -37,6 +37,7 @@ struct SolveParams {
   double eps;
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
+  int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
   int G;                 // CTAs
   int Mb;                // rows per CTA (uniform; last CTAs may own fewer / none)
   int Ns;                // columns per slice owner (multiple of 4)
@@ -224,7 +225,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       }
       it = j + 1;
       // ---- S8: listings' strict relative test (reading C3) ----
-      if (fabs(lam - lam_new) < prm.eps * lam_new || fabs(lam2 - lam_new) < prm.eps * lam_new) break;   // (reading C4b)
+      if (pca_stagnated(lam, lam2, lam_new, prm.eps, prm.test_mode)) break;   // S8 (readings C3, C4b)
       lam2 = lam;
       lam = lam_new;
     }

@@ -211,6 +211,32 @@ def test_golden_worked_examples_on_gpu(binding):
         np.testing.assert_array_equal(got["R"], np.array(g["R_rows"], dtype=np.float32))
 
 
+def test_absolute_test_mode(binding, oracle_mod):
+    """PCA_OPT_TEST_MODE = 1: the text's absolute test |lambda' - lambda| <= eps, on every plan that takes
+    the shape: the hand-derived first-pass values of the worked example, and config 1 against the oracle in the same mode."""
+    g = json.load(open(os.path.join(GOLD, "worked_3x2.json")))
+    a = g["absolute_test"]
+    X = np.asfortranarray(np.array(g["X_rows"], dtype=np.float32))
+    nrm = np.sqrt(a["norm_sq"])
+    for path in (0, 1, 2, 3, 4, 5, 6):
+        got = binding.fit(X, 1, a["eps"], g["max_iter"], inputs.ALGO_NIPALS, center=False, path=path, test_mode=1)
+        assert got["iters"].tolist() == a["iters"], path
+        np.testing.assert_allclose(got["lam"][0], np.sqrt(a["lambda_sq_num"] / a["lambda_sq_den"]), rtol=1e-6)
+        np.testing.assert_allclose(got["P"][:, 0], np.array(a["p_int"]) / nrm, rtol=1e-6)
+        np.testing.assert_allclose(got["T"][:, 0], np.array(a["t_int"]) / nrm, rtol=1e-6)
+    cfg = inputs.config(0)
+    pr = inputs.generate(cfg)
+    Xc = oracle_mod.center(pr.X)
+    eps_abs = 1e-5                                           # ~1e-6 .. 1e-5 relative to the lambdas of config 1 (10 .. 2)
+    ref = oracle_mod.pca(Xc, cfg.K + 1, eps_abs, cfg.max_iter, inputs.ALGO_GS, want_residual=False, test_mode=1)
+    for path in (0, 5, 3, 1):
+        got = binding.fit(pr.X, cfg.K, eps_abs, cfg.max_iter, inputs.ALGO_GS, center=True, path=path, test_mode=1)
+        what = f"absolute test, path {got['info']['path']}"
+        mask = separated_mask(ref.lam, cfg.K)
+        assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
+        assert np.all(np.abs(got["iters"].astype(int) - ref.iters[:cfg.K].astype(int)) <= 3), (got["iters"], ref.iters)
+
+
 def test_degenerate_zero_column_and_zero_matrix(binding, oracle_mod):
     """Reading C7: a component with a zero start column returns lambda = 0, T = P = 0, iters = 0."""
     rng = np.random.default_rng(5)

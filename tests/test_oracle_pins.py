@@ -276,3 +276,33 @@ def test_thread_count_independence(oracle_mod):
         oracle_mod.set_num_threads(n0)
     assert np.array_equal(a.iters, b.iters)
     assert np.array_equal(a.lam, b.lam) and np.array_equal(a.T, b.T) and np.array_equal(a.P, b.P)
+
+
+def test_absolute_test_mode_worked_example(oracle_mod):
+    """The text's absolute test |lambda' - lambda| <= eps (reading C3, non-default mode):
+    hand-derived first-pass values of the 3 x 2 example (lambda starts at 0, so eps >= lambda'_1 stops on pass 1)."""
+    g = json.load(open(os.path.join(GOLD, "worked_3x2.json")))
+    a = g["absolute_test"]
+    X = np.asfortranarray(np.array(g["X_rows"], dtype=np.float64))
+    r = oracle_mod.pca(X, 1, a["eps"], g["max_iter"], oracle_mod.ALGO_NIPALS, test_mode=1)
+    nrm = np.sqrt(a["norm_sq"])
+    assert r.iters.tolist() == a["iters"]
+    np.testing.assert_allclose(r.lam[0] ** 2, a["lambda_sq_num"] / a["lambda_sq_den"], rtol=1e-14)
+    np.testing.assert_allclose(r.P[:, 0], np.array(a["p_int"]) / nrm, rtol=1e-14)
+    np.testing.assert_allclose(r.T[:, 0], np.array(a["t_int"]) / nrm, rtol=1e-14)
+    # the same eps under the listings' relative test runs on (strict test cannot fire on pass 1, reading C8)
+    r0 = oracle_mod.pca(X, 1, 1.0, g["max_iter"], oracle_mod.ALGO_NIPALS, test_mode=0)
+    assert r0.iters.tolist() == g["iters"]
+
+
+def test_absolute_and_relative_tests_agree_when_tight(oracle_mod):
+    """eps_abs = eps_rel * lambda makes the two tests the same decision up to the <= / < boundary: same passes +- 1,
+    same lambda to the convergence error (the choice changes iteration counts, not results)."""
+    cfg = inputs.config(0)
+    pr = inputs.generate(cfg)
+    Xc = oracle_mod.center(pr.X)
+    rel = oracle_mod.pca(Xc, 3, 1e-9, 10000, oracle_mod.ALGO_GS, want_residual=False)
+    for k in range(3):
+        ab = oracle_mod.pca(Xc, k + 1, 1e-9 * rel.lam[k], 10000, oracle_mod.ALGO_GS, want_residual=False, test_mode=1)
+        assert abs(int(ab.iters[k]) - int(rel.iters[k])) <= 1
+        np.testing.assert_allclose(ab.lam[k], rel.lam[k], rtol=1e-8)

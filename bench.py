@@ -355,23 +355,37 @@ def run_cuda_arm(args):
             out["e2e"] = {"value": round(world * K / dt, 3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                           "d2h_bytes_per_step": d2h, "ms_per_step": round(dt * 1e3, 3),
                           "api": "pca_fit_host (pinned host X in; T, P, lambda, iters out)"}
-    # ---- configs[1] measured beside it (cheap: ~10 ms per solve) ----
-    if rank == 0 and not args.no_also and not args.fixed_iters and args.workload != "cfg2":
+    # ---- the other BASELINE.json configs measured beside it (seconds each; `--also cfg2` for configs[1] only) ----
+    if rank == 0 and not args.no_also and not args.fixed_iters:
         del prob
         torch.cuda.empty_cache()
-        c2 = inputs.config(1)
-        p2 = inputs.generate(c2)
-        q = GpuProblem(c2, inputs.ALGO_GS, p2.X)
-        s_ms, r_ms = time_steps(q, 5, 3)
-        roof2, it2 = roofline(q, float(np.mean(r_ms)), peaks)
-        out["also"] = [{"workload": f"BASELINE.json configs[1] {c2.name} K={c2.K} GS-PCA eps={c2.eps:g}",
-                        "value": round(c2.K / (np.mean(s_ms) * 1e-3), 1), "unit": UNIT,
-                        "ms_per_step": round(float(np.mean(s_ms)), 4), "plan": q.ctx.info()["path"],
-                        "us_per_inner_iteration": roof2["us_per_inner_iteration"],
-                        "effective_GBps_vs_hbm": roof2["as_specified_two_read_model"]["GBps"],
-                        "frac_of_hbm_peak": roof2["as_specified_two_read_model"]["frac_of_hbm_peak"],
-                        "bytes_model": "as specified: two reads of R per inner iteration (R is SMEM-resident here)",
-                        "l2": "L2 flushed between steps", "inner_iterations": int(it2.sum())}]
+        out["also"] = []
+        names = [w for w in ("cfg2", "cfg1", "cfg5", "cfg3") if w != args.workload and (args.also == "all" or w in args.also.split(","))]
+        for wname in names:
+            ca = inputs.config(WORKLOADS[wname])
+            pa = inputs.generate(ca)
+            for al in ca.algos if wname == "cfg3" else (pick_algo(ca),):
+                q = GpuProblem(ca, al, pa.X)
+                heavy = 4 * ca.M * ca.N * ca.K > (1 << 34)                  # configs 3 and 5: seconds per solve
+                s_ms, r_ms = time_steps(q, 2 if heavy else 5, 1 if heavy else 3)
+                roofa, ita = roofline(q, float(np.mean(r_ms)), peaks)
+                single_stream = "streaming" in q.ctx.info()["path"]
+                out["also"].append({
+                    "workload": f"BASELINE.json configs[{WORKLOADS[wname]}] {ca.name} K={ca.K} "
+                                f"{'GS-PCA' if al == inputs.ALGO_GS else 'NIPALS-PCA'} eps={ca.eps:g}",
+                    "value": round(ca.K / (np.mean(s_ms) * 1e-3), 1), "unit": UNIT,
+                    "ms_per_step": round(float(np.mean(s_ms)), 4), "plan": q.ctx.info()["path"],
+                    "us_per_inner_iteration": roofa["us_per_inner_iteration"],
+                    "inner_iterations": int(ita.sum()), "hit_max_iter": int((ita >= ca.max_iter).sum()),
+                    "effective_GBps_vs_hbm": roofa["as_specified_two_read_model"]["GBps"],
+                    "frac_of_hbm_peak": roofa["as_specified_two_read_model"]["frac_of_hbm_peak"],
+                    "bytes_model": "as specified: two reads of R per inner iteration" +
+                                   ("" if single_stream else " (R is on chip here: registers)"),
+                    "single_sweep_frac_of_hbm_peak": roofa["frac"] if single_stream else None,
+                    "l2": "input larger than L2" if q.flush is None else "L2 flushed between steps"})
+                del q
+                torch.cuda.empty_cache()
+            del pa
     # ---- cpu_baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline_leg(cfg, algo, pr.X, args.cpu_budget)
@@ -484,6 +498,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true")
+    ap.add_argument("--also", default="all", help="other configs measured beside the workload: all | comma list of cfg1,cfg2,cfg3,cfg5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fig1", action="store_true", help="Fig.-1-shaped sweep (paper's workload) instead of the contract line")
     ap.add_argument("--fig1-sizes", default="512,1024,2048,4096,8192,15000")

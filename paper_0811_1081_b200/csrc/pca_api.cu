@@ -217,6 +217,19 @@ int make_fused_plan(pca_ctx* c, int want) {
     p->off_pc = take(p->cache_pw ? panel : 0);
     p->off_wc = take(p->cache_pw ? panel : 0);
     p->off_slab = take(resident ? (size_t)p->Mb * (size_t)ldr * 4 : 0);
+    // what is left of the shared memory caches the CTA's rows of the first Ksm unit score vectors (GS-PCA, B-partials S6)
+    p->Mbp = (int)round_up(p->Mb, 32);
+    p->Ksm = 0;
+    p->off_vc = (int)off;
+    // (streaming plan: not beyond 100 KB in total -- the sweep keeps 128 KB of loads in flight per SM and those need L1 lines;
+    //  measured on config 4: with all 227 KB as shared memory the sweep is 33 % slower)
+    const long long cap = resident ? (long long)c->smem_optin : (100LL * 1024 < c->smem_optin ? 100LL * 1024 : (long long)c->smem_optin);
+    if (c->algo == PCA_ALGO_GS && (long long)off + 4096 < cap) {
+      long long ks = (cap - (long long)off - 1024) / ((long long)p->Mbp * 4);
+      if (ks > c->K) ks = c->K;
+      ks &= ~1LL;                                                     // pairs of columns
+      if (ks > 0) { p->Ksm = (int)ks; p->off_vc = take((size_t)ks * p->Mbp * 4); }
+    }
     return off;
   };
   auto find = [&](int resident) -> const FusedVariant* {

@@ -68,13 +68,14 @@ struct FusedParams {
   float* Pown;              // [Gs][Ns][Kpad]   owner-private panels P[slice, :], W[slice, :] (W = R^T V) when
   float* Wown;              //                  they do not fit in shared memory (cache_pw == 0)
   int cache_pw;
+  int Ksm, Mbp;             // shared-memory cache of the CTA's rows of the first Ksm unit score vectors: Vc[Ksm][Mbp]
   unsigned* status;         // [0] != 0: an exchange wait gave up (kSpinLimit)
   unsigned* cnt;            // arrival-counter hints of the three hops, 64 words apart (relaxed; see hop_arrive/hop_wait)
   unsigned long long* trace;  // optional phase trace (PCA_OPT_TRACE): [0] = records written, then records
   int trace_cap;              // capacity in records (0 = off)
   // shared-memory carve-up (byte offsets)
   int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_pc, off_wc,
-      off_slab;
+      off_slab, off_vc;
 };
 
 constexpr int kRB = 4;   // rows per batch
@@ -323,6 +324,113 @@ __device__ __forceinline__ void hop_wait(const unsigned* ctr, unsigned expected,
   __syncthreads();
 }
 
+// ------------------------------------------------------------------------------------ LL words, generic addresses
+// Same protocol as pca_fused.cuh ("LL exchange"), but through GENERIC addresses: when the whole problem runs in ONE CTA
+// the exchange buffers are placed in shared memory (the warps of the CTA exchange through them exactly as CTAs do through
+// L2, at shared-memory latency), otherwise they are the global buffers of the workspace.
+__device__ __forceinline__ void gl_st2(u64* p, u64 a, u64 b) {
+  asm volatile("st.relaxed.gpu.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+__device__ __forceinline__ void gl_ld2(const u64* p, u64& a, u64& b) {
+  asm volatile("ld.relaxed.gpu.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void gl_st2d(u64* p, double v, unsigned seq) {
+  const u64 bits = (u64)__double_as_longlong(v);
+  gl_st2(p, ll_word((unsigned)bits, seq), ll_word((unsigned)(bits >> 32), seq));
+}
+__device__ __forceinline__ void gl_wait2(const u64* p, unsigned seq, u64& a, u64& b, unsigned* status) {
+  unsigned spins = 0;
+  while ((unsigned)(a >> 32) != seq || (unsigned)(b >> 32) != seq) {
+    gl_ld2(p, a, b);
+    if (++spins > kSpinLimit) { *status = 1u; break; }
+  }
+}
+
+// Owner-side combination of one exchange region: rows of `stride` words, one row per part (= producing CTA), of which the
+// first 2*hp words (hp pairs, hp a power of two <= kThreads) are summed over the nparts rows in fp64:
+//   out[2*pair], out[2*pair+1] = sum_parts row[part][2*pair], row[part][2*pair+1]          (pairs >= npairs are skipped)
+// Thread t owns pair t % hp and the parts t / hp + i * (kThreads / hp) (a warp reads contiguous pairs of a row: coalesced
+// 16-byte loads, up to INF in flight per thread), sums them in ascending order, then the threads of a pair are combined
+// by shuffles (inside a warp) and through `red` (kThreads double2, across warps) in a fixed order.  If f64_pair0, pair 0
+// holds ONE fp64 value.  Two-phase so that two regions can be in flight at once: *_issue, *_finish.
+struct RegGather {
+  const u64* base;
+  int stride, hp, npairs, nparts;
+  bool f64_pair0;
+  double2* red;       // kThreads entries
+  double* out;
+};
+
+template <int INF>
+__device__ __forceinline__ void reg_gather_issue(const RegGather& gq, u64 (&x)[INF], u64 (&y)[INF]) {
+  const int tid = threadIdx.x;
+  const int pair = tid & (gq.hp - 1), pslot = tid / gq.hp, pstep = kThreads / gq.hp;
+#pragma unroll
+  for (int i = 0; i < INF; ++i) {
+    const int part = pslot + i * pstep;
+    x[i] = 0; y[i] = 0;
+    if (part < gq.nparts && pair < gq.npairs) gl_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
+  }
+}
+
+template <int INF>
+__device__ __forceinline__ void reg_gather_finish(const RegGather& gq, u64 (&x)[INF], u64 (&y)[INF], unsigned seq, unsigned* status) {
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int hp = gq.hp;
+  const int pair = tid & (hp - 1), pslot = tid / hp, pstep = kThreads / hp;
+  const bool f64 = gq.f64_pair0 && pair == 0;
+  double a0 = 0.0, a1 = 0.0;
+  if (pair < gq.npairs) {
+#pragma unroll
+    for (int i = 0; i < INF; ++i) {
+      const int part = pslot + i * pstep;
+      if (part < gq.nparts) {
+        gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
+        if (f64) a0 += ll_d(x[i], y[i]);
+        else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
+      }
+    }
+    for (int p0 = pslot + INF * pstep; p0 < gq.nparts; p0 += INF * pstep) {     // more parts than one batch covers
+#pragma unroll
+      for (int i = 0; i < INF; ++i) {
+        const int part = p0 + i * pstep;
+        x[i] = 0; y[i] = 0;
+        if (part < gq.nparts) gl_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
+      }
+#pragma unroll
+      for (int i = 0; i < INF; ++i) {
+        const int part = p0 + i * pstep;
+        if (part < gq.nparts) {
+          gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
+          if (f64) a0 += ll_d(x[i], y[i]);
+          else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
+        }
+      }
+    }
+  }
+  for (int o = 16; o >= hp; o >>= 1) {                                        // lanes l and l ^ o own the same pair when o >= hp
+    a0 += __shfl_xor_sync(0xffffffffu, a0, o);
+    a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+  }
+  if (hp >= 32) gq.red[tid] = make_double2(a0, a1);
+  else if (lane < hp) gq.red[w * hp + lane] = make_double2(a0, a1);
+}
+
+// after a __syncthreads(): threads < hp write the sums
+__device__ __forceinline__ void reg_gather_store(const RegGather& gq) {
+  const int t = threadIdx.x, hp = gq.hp;
+  if (t < hp && t < gq.npairs) {
+    const int nslots = hp >= 32 ? kThreads / hp : kWarps;
+    double a0 = 0.0, a1 = 0.0;
+    for (int sl = 0; sl < nslots; ++sl) {
+      const double2 v = gq.red[sl * hp + t];
+      a0 += v.x; a1 += v.y;
+    }
+    gq.out[2 * t] = a0;
+    gq.out[2 * t + 1] = a1;
+  }
+}
+
 // One reduction job: out[j] = sum over parts b < nparts of word (base + b*stride)[j], j < 2*units, fp64, fixed order
 // (lane l takes parts l, l+32, ... in order, then a shuffle tree).  If f64_unit0, words 0-1 hold one fp64 value.
 struct LLJob {
@@ -419,6 +527,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
   double* praw_s = reinterpret_cast<double*>(smem + prm.off_praw);// Ns: p~ / p^ slice of this owner
   float* lam_s = reinterpret_cast<float*>(smem + prm.off_lam);    // Kpad
   float* slab = reinterpret_cast<float*>(smem + prm.off_slab);    // resident: Mb x ldr
+  float* Vc = reinterpret_cast<float*>(smem + prm.off_vc);        // Ksm x Mbp: cached unit score rows (GS-PCA)
 
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
@@ -505,7 +614,24 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         jq.nparts = G; jq.stride = Ns; jq.f64_unit0 = false;
         jsb.base = prm.SBx + (size_t)par * G * SBw; jsb.out = sb_s; jsb.units = 1 + ((gsk && !first) ? ((k + 1) >> 1) : 0);
         jsb.nparts = G; jsb.stride = SBw; jsb.f64_unit0 = true;
-        ll_reduce2(jsb, jq, seq, status);
+        if (jsb.units <= 16) {
+          ll_reduce2(jsb, jq, seq, status);
+        } else {
+          // many B units: lanes over the units of a part (contiguous words), parts in turn, instead of a warp per unit with
+          // lanes over parts 1 KB apart (measured on config 4 at k = 127: this phase and hop 2 were 10 us each)
+          RegGather gsb;
+          int hs = 32;
+          while (hs < jsb.units) hs <<= 1;
+          gsb.base = jsb.base; gsb.stride = SBw; gsb.hp = hs; gsb.npairs = jsb.units; gsb.nparts = G; gsb.f64_pair0 = true;
+          gsb.red = reinterpret_cast<double2*>(qs); gsb.out = sb_s;
+          u64 sx[8], sy[8];
+          reg_gather_issue<8>(gsb, sx, sy);
+          jsb.units = 0;
+          ll_reduce2(jsb, jq, seq, status);                                   // the owner's q slice, meanwhile
+          reg_gather_finish<8>(gsb, sx, sy, seq, status);
+          __syncthreads();
+          reg_gather_store(gsb);
+        }
       }
       __syncthreads();
       trace_mark(prm, tn, TR_X1);
@@ -571,12 +697,24 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         e2 += (unsigned)Gs;
         hop_wait(cnt2, e2, status);
         // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
-        {
+        if (k <= 30) {
           LLJob ja, jn;
           ja.base = prm.Ax + (size_t)par * Gs * Kpad; ja.out = A_s; ja.units = (k + 1) >> 1; ja.nparts = Gs; ja.stride = Kpad;
           ja.f64_unit0 = false;
           jn = ja; jn.units = 0;
           ll_reduce2(ja, jn, seq, status);
+        } else {
+          RegGather ga;
+          const int ua = (k + 1) >> 1;
+          int ha = 32;
+          while (ha < ua) ha <<= 1;
+          ga.base = prm.Ax + (size_t)par * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
+          ga.f64_pair0 = false; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
+          u64 ax8[8], ay8[8];
+          reg_gather_issue<8>(ga, ax8, ay8);
+          reg_gather_finish<8>(ga, ax8, ay8, seq, status);
+          __syncthreads();
+          reg_gather_store(ga);
         }
         __syncthreads();
         trace_mark(prm, tn, TR_X2);
@@ -654,15 +792,27 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           ll_st2d(sbx, a, seq);
         }
         if (gsk) {                                                            // S6: B-partials V^T t~
+          // the CTA's rows of the first Ksm unit score vectors are cached in shared memory (Vc, column-major), the rest
+          // comes from T in global memory (L2)
           for (int j0 = 2 * w; j0 < k; j0 += 2 * kWarps) {
-            const float* v0 = Tb + (size_t)j0 * M;
-            const float* v1 = v0 + M;
             const bool two = j0 + 1 < k;
             float a0 = 0.f, a1 = 0.f;
-            for (int i = lane; i < mb; i += 32) {
-              const float tt = ttil_s[i];
-              a0 = fmaf(v0[i], tt, a0);
-              if (two) a1 = fmaf(v1[i], tt, a1);
+            if (j0 + 1 < prm.Ksm) {
+              const float* c0 = Vc + (size_t)j0 * prm.Mbp;
+              const float* c1 = c0 + prm.Mbp;
+              for (int i = lane; i < mb; i += 32) {
+                const float tt = ttil_s[i];
+                a0 = fmaf(c0[i], tt, a0);
+                if (two) a1 = fmaf(c1[i], tt, a1);
+              }
+            } else {
+              const float* v0 = Tb + (size_t)j0 * M;
+              const float* v1 = v0 + M;
+              for (int i = lane; i < mb; i += 32) {
+                const float tt = ttil_s[i];
+                a0 = fmaf(v0[i], tt, a0);
+                if (two) a1 = fmaf(v1[i], tt, a1);
+              }
             }
             const double s0 = warp_sum((double)a0), s1 = warp_sum((double)a1);
             if (lane == 0) ll_st2(sbx + 2 + j0, ll_wordf((float)s0, seq), ll_wordf((float)s1, seq));
@@ -676,7 +826,10 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
 
     // ---- component done ----
     if (degenerate) {
-      for (int i = tid; i < mb; i += kThreads) { Tb[(size_t)k * M + i] = 0.f; d_s[i] = 0.f; }
+      for (int i = tid; i < mb; i += kThreads) {
+        Tb[(size_t)k * M + i] = 0.f; d_s[i] = 0.f;
+        if (gs && k < prm.Ksm) Vc[(size_t)k * prm.Mbp + i] = 0.f;
+      }
       if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = 0.f;
       if (tid < Ns) { Pc[(size_t)tid * Kpad + k] = 0.f; Wc[(size_t)tid * Kpad + k] = 0.f; }
       for (int n = tid; n < ldr; n += kThreads) pdef_s[n] = 0.f;
@@ -695,6 +848,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         }
         d_s[i] = t;                                                           // R -= lambda v p^T  /  R -= t p^T
         Tb[(size_t)k * M + i] = gs ? t * inv : t;
+        if (gs && k < prm.Ksm) Vc[(size_t)k * prm.Mbp + i] = t * inv;
       }
       if (tid < ns) {
         const float pk = p_s[n0 + tid];

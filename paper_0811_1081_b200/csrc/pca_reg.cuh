@@ -80,28 +80,6 @@ __device__ __forceinline__ void reg_trace(const RegParams& prm, int& tn, int pha
   }
 }
 
-// ------------------------------------------------------------------------------------ LL words, generic addresses
-// Same protocol as pca_fused.cuh ("LL exchange"), but through GENERIC addresses: when the whole problem runs in ONE CTA
-// the exchange buffers are placed in shared memory (the warps of the CTA exchange through them exactly as CTAs do through
-// L2, at shared-memory latency), otherwise they are the global buffers of the workspace.
-__device__ __forceinline__ void gl_st2(u64* p, u64 a, u64 b) {
-  asm volatile("st.relaxed.gpu.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
-}
-__device__ __forceinline__ void gl_ld2(const u64* p, u64& a, u64& b) {
-  asm volatile("ld.relaxed.gpu.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
-}
-__device__ __forceinline__ void gl_st2d(u64* p, double v, unsigned seq) {
-  const u64 bits = (u64)__double_as_longlong(v);
-  gl_st2(p, ll_word((unsigned)bits, seq), ll_word((unsigned)(bits >> 32), seq));
-}
-__device__ __forceinline__ void gl_wait2(const u64* p, unsigned seq, u64& a, u64& b, unsigned* status) {
-  unsigned spins = 0;
-  while ((unsigned)(a >> 32) != seq || (unsigned)(b >> 32) != seq) {
-    gl_ld2(p, a, b);
-    if (++spins > kSpinLimit) { *status = 1u; break; }
-  }
-}
-
 // ------------------------------------------------------------------------------------ row reduction
 // Eight values per lane, summed over the SEG lanes of a segment (SEG = 8, 16 or 32, a power of two).
 // The first three butterfly steps halve the number of values instead of duplicating sums, so that
@@ -315,91 +293,6 @@ __device__ __forceinline__ void reg_ll_reduce_all(const u64* base, int stride, i
       reg_ll_unit<5>(base + (size_t)u * ustride, stride, nparts, 0, false, seq, status, a0, a1);
       if (lane == 0) { out[2 * u] = a0; out[2 * u + 1] = a1; }
     }
-  }
-}
-
-// Owner-side combination of one exchange region: rows of `stride` words, one row per part (= producing CTA), of which the
-// first 2*hp words (hp pairs, hp a power of two <= kThreads) are summed over the nparts rows in fp64:
-//   out[2*pair], out[2*pair+1] = sum_parts row[part][2*pair], row[part][2*pair+1]          (pairs >= npairs are skipped)
-// Thread t owns pair t % hp and the parts t / hp + i * (kThreads / hp) (a warp reads contiguous pairs of a row: coalesced
-// 16-byte loads, up to INF in flight per thread), sums them in ascending order, then the threads of a pair are combined
-// by shuffles (inside a warp) and through `red` (kThreads double2, across warps) in a fixed order.  If f64_pair0, pair 0
-// holds ONE fp64 value.  Two-phase so that two regions can be in flight at once: *_issue, *_finish.
-struct RegGather {
-  const u64* base;
-  int stride, hp, npairs, nparts;
-  bool f64_pair0;
-  double2* red;       // kThreads entries
-  double* out;
-};
-
-template <int INF>
-__device__ __forceinline__ void reg_gather_issue(const RegGather& gq, u64 (&x)[INF], u64 (&y)[INF]) {
-  const int tid = threadIdx.x;
-  const int pair = tid & (gq.hp - 1), pslot = tid / gq.hp, pstep = kThreads / gq.hp;
-#pragma unroll
-  for (int i = 0; i < INF; ++i) {
-    const int part = pslot + i * pstep;
-    x[i] = 0; y[i] = 0;
-    if (part < gq.nparts && pair < gq.npairs) gl_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
-  }
-}
-
-template <int INF>
-__device__ __forceinline__ void reg_gather_finish(const RegGather& gq, u64 (&x)[INF], u64 (&y)[INF], unsigned seq, unsigned* status) {
-  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  const int hp = gq.hp;
-  const int pair = tid & (hp - 1), pslot = tid / hp, pstep = kThreads / hp;
-  const bool f64 = gq.f64_pair0 && pair == 0;
-  double a0 = 0.0, a1 = 0.0;
-  if (pair < gq.npairs) {
-#pragma unroll
-    for (int i = 0; i < INF; ++i) {
-      const int part = pslot + i * pstep;
-      if (part < gq.nparts) {
-        gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
-        if (f64) a0 += ll_d(x[i], y[i]);
-        else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
-      }
-    }
-    for (int p0 = pslot + INF * pstep; p0 < gq.nparts; p0 += INF * pstep) {     // more parts than one batch covers
-#pragma unroll
-      for (int i = 0; i < INF; ++i) {
-        const int part = p0 + i * pstep;
-        x[i] = 0; y[i] = 0;
-        if (part < gq.nparts) gl_ld2(gq.base + (size_t)part * gq.stride + 2 * pair, x[i], y[i]);
-      }
-#pragma unroll
-      for (int i = 0; i < INF; ++i) {
-        const int part = p0 + i * pstep;
-        if (part < gq.nparts) {
-          gl_wait2(gq.base + (size_t)part * gq.stride + 2 * pair, seq, x[i], y[i], status);
-          if (f64) a0 += ll_d(x[i], y[i]);
-          else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
-        }
-      }
-    }
-  }
-  for (int o = 16; o >= hp; o >>= 1) {                                        // lanes l and l ^ o own the same pair when o >= hp
-    a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-    a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-  }
-  if (hp >= 32) gq.red[tid] = make_double2(a0, a1);
-  else if (lane < hp) gq.red[w * hp + lane] = make_double2(a0, a1);
-}
-
-// after a __syncthreads(): threads < hp write the sums
-__device__ __forceinline__ void reg_gather_store(const RegGather& gq) {
-  const int t = threadIdx.x, hp = gq.hp;
-  if (t < hp && t < gq.npairs) {
-    const int nslots = hp >= 32 ? kThreads / hp : kWarps;
-    double a0 = 0.0, a1 = 0.0;
-    for (int sl = 0; sl < nslots; ++sl) {
-      const double2 v = gq.red[sl * hp + t];
-      a0 += v.x; a1 += v.y;
-    }
-    gq.out[2 * t] = a0;
-    gq.out[2 * t + 1] = a1;
   }
 }
 

@@ -73,7 +73,8 @@ enum {
 /* Phase ids of the trace records (pca_trace).  One inner pass of the single-sweep kernel is
  * PREADY -> SWEEP -> PUBLISHED -> X1 -> TEST -> QSLICE -> [APART -> X2 ->] PHAT -> X3 -> PREADY. */
 enum {
-  PCA_TR_COMPONENT = 1, /* component k starts (S1) */
+  PCA_TR_COMPONENT = 1, /* component k starts (S1)   (path 5 emits the subset COMPONENT, LOADS_DONE, X1, TEST, X2, PHAT, X3, SWEEP,
+                           PUBLISHED, FINAL of these ids) */
   PCA_TR_LOADS_DONE = 2,/* first sweep of the component done: pending deflation S9 + q = R^T t0 (S2), published */
   PCA_TR_X1 = 3,        /* grid barrier 1 passed: all partial raw loads / |t~|^2 / B-partials visible */
   PCA_TR_TEST = 4,      /* lambda' (S7) and the convergence test (S8) taken */
@@ -163,12 +164,16 @@ int pca_run(pca_ctx*, const float* X, float* T, float* P, float* lambda, int32_t
  * this context has completed ("return T, P, R"). */
 int pca_residual(const pca_ctx*, const float** R);
 
-/* Device-side phase trace of the last pca_run (tracing aid; PCA_OPT_TRACE > 0, single-sweep kernel).
- *   records   dev pointer inside the workspace: records[0] = number of records written (<= capacity),
- *             records[1 + i] = (phase id << 56) | (SM cycle counter of CTA 0 & (2^56 - 1)), in program order
+/* Device-side phase trace of the last pca_run (tracing aid; PCA_OPT_TRACE > 0, single-sweep kernels, paths 3-5).
+ *   records   dev pointer inside the workspace: records[0] = number of records written per slot,
+ *             records[1 + i] = (phase id << 56) | (time stamp & (2^56 - 1)), in program order.
+ *             paths 3, 4: ONE slot, CTA 0, time stamp = its SM cycle counter (clock64);
+ *             path 5: one slot per CTA (CTA b owns records [b*capacity/G, (b+1)*capacity/G)), time stamp = %globaltimer
+ *             in ns (common to all SMs), so that the timelines of the CTAs can be laid side by side.
+ *             (With PCA_OPT_TRACE > 0 the auto plan does not pick the one-CTA kernel, which has no trace.)
  *   capacity  the PCA_OPT_TRACE value
  * Valid after the stream of pca_run has been synchronised; the caller copies it to the host.
- * Errors: PCA_EINVAL, PCA_EUNSUPPORTED (trace off or two-sweep kernel), PCA_EWORKSPACE (no run yet). */
+ * Errors: PCA_EINVAL, PCA_EUNSUPPORTED (trace off, or a kernel without trace), PCA_EWORKSPACE (no run yet). */
 int pca_trace(const pca_ctx*, const uint64_t** records, int64_t* capacity);
 
 /* Convenience entry with HOST buffers (used for end-to-end timing): copies X (host, M x N,

@@ -342,7 +342,6 @@ int make_reg_plan(pca_ctx* c) {
     p.off_A = take((size_t)(2 + p.Kpad) * 8);
     p.off_scr = take((size_t)pca::kThreads * 8);
     p.off_praw = take((size_t)2 * p.Ns * 8);
-    p.off_bred = take((size_t)pca::kThreads * 4);
     const size_t KV = (size_t)(p.Kpad | 1);                           // odd row stride (bank-conflict-free both ways)
     p.off_vb = take(gs ? rows * KV * 4 : 0);
     p.off_pc = take(gs ? (size_t)p.Ns * KV * 4 : 0);

@@ -58,7 +58,7 @@ struct RegParams {
   unsigned long long* trace;
   int trace_cap;
   // shared-memory carve-up (byte offsets)
-  int off_p, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_bred, off_vb, off_pc, off_wc;
+  int off_p, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_vb, off_pc, off_wc;
   int off_x;             // >= 0 (one CTA only): the exchange buffers live in shared memory at this offset
 };
 

@@ -235,7 +235,7 @@ def to_colmajor(t):
 
 
 def fit(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, path=PCA_PATH_AUTO, ctas=0,
-        want_residual=False, test_mode=0):
+        want_residual=False, test_mode=0, options=None):
     """One-call helper used by tests / smoke: numpy (M, N) float32 in -> dict of numpy results.
 
     Runs pca_center (optional) and pca_run on the GPU through the C ABI."""
@@ -248,6 +248,8 @@ def fit(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, path=P
         ctx.pca_set_option(PCA_OPT_CTAS, ctas)
     if test_mode:
         ctx.pca_set_option(PCA_OPT_TEST_MODE, test_mode)
+    for opt, val in (options or {}).items():
+        ctx.pca_set_option(opt, val)
     X = from_colmajor(X_np)
     if center:
         ctx.pca_center(X)

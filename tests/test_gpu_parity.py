@@ -154,6 +154,34 @@ def test_paper_workload_uniform(binding, oracle_mod, algo):
     assert abs(e_g - e_o) <= 1e-3 * e_o, f"{what} captured energy {e_g} vs {e_o}"
 
 
+@pytest.mark.parametrize("owners,kdirect", [(4, 0), (16, 6), (32, 30), (8, 14)])
+def test_register_kernel_exchange_options(binding, oracle_mod, owners, kdirect):
+    """The register-resident kernel's exchange shape is tunable (PCA_OPT_OWNERS, PCA_OPT_KDIRECT): fewer / more slice owners,
+    B combined directly by the owners (k <= kdirect) or in two levels.  Every setting is the same arithmetic in another
+    summation order: parity with the oracle must hold for all of them (the defaults are what the other tests run)."""
+    cfg = inputs.scaled(inputs.config(1), 3000, 700, K=40)
+    pr = inputs.generate(cfg)
+    Xc, ref = _oracle_run(oracle_mod, pr.X, cfg, inputs.ALGO_GS, K=cfg.K)
+    got = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, center=True, path=5, want_residual=True,
+                      options={binding.PCA_OPT_OWNERS: owners, binding.PCA_OPT_KDIRECT: kdirect})
+    what = f"{cfg.name} owners={got['info']['owners']} kdirect={kdirect}"
+    assert got["info"]["owners"] == owners
+    mask = separated_mask(ref.lam, cfg.K)
+    assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
+    _check_invariants(got, f64(got["Xc"]), inputs.ALGO_GS, cfg.K, what)
+
+
+def test_one_cta_kernel_is_deterministic_and_matches_register_kernel(binding):
+    cfg = inputs.scaled(inputs.config(0), 256, 64, K=8)
+    pr = inputs.generate(cfg)
+    a = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=6)
+    b = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=6)
+    c = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=5)
+    for key in ("T", "P", "lam", "iters"):
+        np.testing.assert_array_equal(a[key], b[key])
+    np.testing.assert_allclose(a["lam"], c["lam"], rtol=1e-5)
+
+
 def test_paths_agree_and_are_deterministic(binding):
     """Resident and streaming plans run the same arithmetic in the same order per CTA count;
     each plan is bitwise reproducible run to run (fixed-order reductions)."""

@@ -182,6 +182,33 @@ def test_one_cta_kernel_is_deterministic_and_matches_register_kernel(binding):
     np.testing.assert_allclose(a["lam"], c["lam"], rtol=1e-5)
 
 
+@pytest.mark.parametrize("ci,K,reps", [(1, 32, 25), (0, 8, 50)])
+def test_repeated_full_size_runs_are_bitwise_identical(binding, ci, K, reps):
+    """Stress of the barrier-free exchange protocol at the sizes bench.py times (configs 2 and 1): the same context run
+    again and again must give bitwise identical T, P, lambda, iters and a clean run-status word every time."""
+    import torch
+    cfg = inputs.config(ci)
+    pr = inputs.generate(cfg)
+    ctx = binding.PcaContext(cfg.M, cfg.N, K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+    X = binding.from_colmajor(pr.X)
+    ctx.pca_center(X)
+    T = torch.empty((K, cfg.M), device="cuda")
+    P = torch.empty((K, cfg.N), device="cuda")
+    lam = torch.empty(K, device="cuda")
+    it = torch.empty(K, dtype=torch.int32, device="cuda")
+    ref = None
+    for r in range(reps):
+        ctx.pca_run(X, T, P, lam, it)
+        torch.cuda.synchronize()
+        assert ctx.pca_get_info(binding.PCA_INFO_RUN_STATUS) == 0, f"run {r}: an exchange wait gave up"
+        cur = (T.clone(), P.clone(), lam.clone(), it.clone())
+        if ref is None:
+            ref = cur
+        for a, b in zip(ref, cur):
+            assert torch.equal(a, b), f"run {r} differs from run 0"
+    ctx.pca_destroy()
+
+
 def test_paths_agree_and_are_deterministic(binding):
     """Resident and streaming plans run the same arithmetic in the same order per CTA count;
     each plan is bitwise reproducible run to run (fixed-order reductions)."""

@@ -33,8 +33,11 @@
 //
 // Parity pins (tests/test_oracle_pins.py): prescribed spectrum (noise-free), Jacobi on X^T X,
 // numpy SVD, energy identity, decomposition identity eq. (4), orthogonality, hand-derived
-// worked examples under tests/golden/, control-flow special cases.  No function here is
-// "parity unpinned".
+// worked examples under tests/golden/ (NIPALS 3x2, GS-PCA 3x3 with one pass per component), control-
+// flow special cases.  tests/test_oracle_mutants.py types one plausible mistake at a time into a
+// copy of this file (wrong sign / dropped step / k-1 columns in either Gram-Schmidt step, undeflated
+// start vector, eps scaled by the old lambda, ...) and checks that a pin fails for each.  No function
+// here is "parity unpinned".
 //
 // Layout everywhere: column-major, leading dimension = number of rows, the paper's
 // id(m,n,ld) = n*ld + m.

@@ -38,7 +38,9 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        lib = ctypes.CDLL(build())
+        # PCA_ORACLE_LIB: tests/test_oracle_mutants.py points this at a deliberately broken build of pca_oracle.cpp to
+        # check that the pins notice (mutation test of the pins); never set otherwise.
+        lib = ctypes.CDLL(os.environ.get("PCA_ORACLE_LIB") or build())
         i64, f64, i32 = ctypes.c_int64, ctypes.c_double, ctypes.c_int
         dp = ctypes.POINTER(ctypes.c_double)
         ip = ctypes.POINTER(ctypes.c_int32)

@@ -8,9 +8,10 @@ the double-precision oracle (oracle/pca_oracle.cpp, the paper's algorithm step b
 on the FULL-SIZE seeded input for the first K_s components.  Components are extracted one after
 the other, so the first K_s components of a K-component solve are exactly the
 K_s-component solve: the stored prefix is what the full run would return for those components.
-K_s is the whole K where the oracle finishes in a minute (configs 1, 2) and a short prefix where
-one oracle pass streams 0.5-1 GiB (configs 3, 4) or K is large (config 5); one extra component
-is run so that the separation of component K_s - 1 from its successor is known.
+K_s is the whole K for configs 1-4 (configs 3 and 4: one oracle pass streams 1-2 GiB, the full
+solves take tens of minutes on 8 cores and are run once, here, in the CPU container) and a prefix
+for config 5 (K = N = 512, ~270 k passes); one extra component is run so that the separation of
+component K_s - 1 from its successor is known.
 
 Output: tests/golden/oracle_<cfg>_<algo>.npz with
     lam      (K_s + 1,) float64   lambda_k
@@ -19,6 +20,10 @@ Output: tests/golden/oracle_<cfg>_<algo>.npz with
     rows     (S,) int64           sampled row indices (np.linspace over [0, M-1])
     T_rows   (S, K_s + 1) float32 the scores at those rows
     x_fro2   float64              ||X_c||_F^2 of the centred input the oracle saw
+    x_idx    (64,) int64          flat column-major indices into the RAW (uncentred) float32 input
+    x_val    (64,) float32        the raw input at those indices: the tests assert that the regenerated
+                                  input still IS the matrix the oracle saw (inputs.py draws U, V with a
+                                  LAPACK QR; a different LAPACK could rotate the basis silently)
     meta     json string          config, K_s, seed, eps, max_iter, wall seconds, this command
 The GPU parity tests (tests/test_gpu_parity.py) regenerate the same seeded input, run the CUDA
 path at full size and compare against these values (tolerances of BASELINE.json's north_star).
@@ -41,7 +46,8 @@ import oracle  # noqa: E402
 from paper_0811_1081_b200 import inputs  # noqa: E402
 
 # components of the full-size solve that are stored (K_s); the run itself does K_s + 1
-PREFIX = {0: 8, 1: 32, 2: 4, 3: 8, 4: 16}
+PREFIX = {0: 8, 1: 32, 2: 64, 3: 128, 4: 16}
+X_SAMPLES = 64
 SAMPLED_ROWS = 256
 
 
@@ -55,6 +61,9 @@ def make(ci: int) -> None:
     krun = min(ks + 1, cfg.N)
     t0 = time.time()
     pr = inputs.generate(cfg)
+    x_idx = np.unique(np.linspace(0, cfg.M * cfg.N - 1, X_SAMPLES).astype(np.int64))
+    x_val = pr.X.ravel(order="K")[x_idx].copy()                      # pr.X is Fortran-ordered: memory order = column-major
+    assert pr.X.flags.f_contiguous
     Xc = oracle.center(pr.X)
     del pr
     x_fro2 = float(np.sum(Xc * Xc))
@@ -69,7 +78,7 @@ def make(ci: int) -> None:
                     command=f"python tests/golden/make_oracle_prefix.py {ci}")
         np.savez_compressed(out_path(cfg, algo), lam=r.lam, iters=r.iters, P=r.P.astype(np.float32),
                             rows=rows, T_rows=r.T[rows, :].astype(np.float32), x_fro2=np.float64(x_fro2),
-                            meta=json.dumps(meta))
+                            x_idx=x_idx, x_val=x_val, meta=json.dumps(meta))
         print(f"{cfg.name} algo {algo}: K_run {krun} iters {r.iters.tolist()} lam[:4] {r.lam[:4]} "
               f"oracle {wall:.1f}s (gen+centre {t1 - t0:.1f}s)", flush=True)
 

@@ -306,3 +306,87 @@ def test_absolute_and_relative_tests_agree_when_tight(oracle_mod):
         ab = oracle_mod.pca(Xc, k + 1, 1e-9 * rel.lam[k], 10000, oracle_mod.ALGO_GS, want_residual=False, test_mode=1)
         assert abs(int(ab.iters[k]) - int(rel.iters[k])) <= 1
         np.testing.assert_allclose(ab.lam[k], rel.lam[k], rtol=1e-8)
+
+
+# ----------------------------------------------------------------------------- round-2 pins
+def test_golden_worked_gs_3x3_one_pass(oracle_mod):
+    """Hand-derived GS-PCA example (tests/golden/worked_gs_3x3.json): K = 2, max_iter = 1.  Component 1 depends on the start vector
+    being column 1 of the DEFLATED residual and on a non-zero scores-side coefficient B (:1030-1031)."""
+    g = json.load(open(os.path.join(GOLD, "worked_gs_3x3.json")))
+    X = np.array(g["X_rows"], dtype=np.float64)
+    r = oracle_mod.pca(X, g["K"], g["eps"], g["max_iter"], oracle_mod.ALGO_GS)
+    assert list(r.iters) == g["iters"]
+    for k in range(2):
+        num, den = g["lambda_sq"][k]
+        np.testing.assert_allclose(r.lam[k] ** 2, num / den, rtol=1e-14)
+        np.testing.assert_allclose(r.P[:, k], np.array(g["P_int"][k]) / math.sqrt(g["P_norm_sq"][k]), rtol=0, atol=1e-15)
+        np.testing.assert_allclose(r.T[:, k], np.array(g["T_int"][k]) / math.sqrt(g["T_den_sq"][k]), rtol=0, atol=2e-15)
+    np.testing.assert_allclose(r.R, np.array(g["R_num"], dtype=np.float64) / np.array(g["R_den"], dtype=np.float64), rtol=0, atol=2e-15)
+    # what the two plausible mistakes would have produced instead (same derivation): far outside the tolerance above
+    num, den = g["mutants"]["no_scores_projection_lambda1_sq"]
+    assert abs(r.lam[1] ** 2 - num / den) > 1e-1
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_gs_loads_projection_is_needed_after_one_pass(oracle_mod, seed):
+    """The loads-side Gram-Schmidt step A = P_(k)^T p, p -= P_(k) A.  After >= 2 passes R^T t is
+    orthogonal to the previous loadings to rounding anyway, so only an EARLY-STOPPED run sees the step: with max_iter = 1 the
+    deflation leaves R p_1 = V_(1) B != 0, the raw loads of component 2 have a component along p_1 of order 1e-2, and the claim
+    'orthogonal loads' holds only because of this step (a dropped step, a wrong sign or k-1 columns all
+    give max|P^T P - I| ~ 1e-2)."""
+    rng = np.random.default_rng(100 + seed)
+    X = rng.standard_normal((6, 4))
+    r = oracle_mod.pca(X, 3, 1e-7, 1, oracle_mod.ALGO_GS)
+    assert list(r.iters) == [1, 1, 1]
+    assert np.max(np.abs(r.P.T @ r.P - np.eye(3))) <= 1e-12
+    Vn = r.T / r.lam[None, :]
+    assert np.max(np.abs(Vn.T @ Vn - np.eye(3))) <= 1e-12
+    # the raw loads of component 2 are NOT orthogonal to p_1: recompute them from the returned quantities
+    # (R_2 = X - T_(2) P_(2)^T by eq. (4), PAPER.md:42; start vector = column 2 of R_2, PAPER.md:1017)
+    R2 = X - r.T[:, :2] @ r.P[:, :2].T
+    p_raw = R2.T @ R2[:, 2]
+    assert abs(r.P[:, 1] @ p_raw) / np.linalg.norm(p_raw) > 1e-4
+    # eq. (4) still holds elementwise
+    np.testing.assert_allclose(r.T @ r.P.T + r.R, X, rtol=0, atol=1e-13)
+
+
+def test_relative_test_scales_eps_with_the_newest_lambda(oracle_mod):
+    """`fabs(a-b) < er*b` with b the NEWEST lambda': on the 3 x 2 example lambda = 0 before pass 1, so
+    with eps = 2 the test |0 - lambda'| = lambda' < 2 lambda' fires on pass 1.  Scaling with the OLD lambda (= 0) could not."""
+    g = json.load(open(os.path.join(GOLD, "worked_3x2.json")))
+    X = np.array(g["X_rows"], dtype=np.float64)
+    for algo in (oracle_mod.ALGO_NIPALS, oracle_mod.ALGO_GS):
+        r = oracle_mod.pca(X, 1, 2.0, g["max_iter"], algo)
+        assert list(r.iters) == [1]
+        np.testing.assert_allclose(r.lam[0] ** 2, g["lambda_pass1_sq_num"] / g["lambda_pass1_sq_den"], rtol=1e-14)
+
+
+def test_start_vector_is_the_deflated_column_numeric(oracle_mod):
+    """Reading C6 on a random matrix with max_iter = 1: the loadings of component 1 are
+    R_1^T R_1[:,1] normalised (R_1 = X - t_0 p_0^T, eq. 3), NOT R_1^T X[:,1]."""
+    rng = np.random.default_rng(21)
+    X = rng.standard_normal((7, 5))
+    r = oracle_mod.pca(X, 2, 1e-7, 1, oracle_mod.ALGO_NIPALS)
+    R1 = X - np.outer(r.T[:, 0], r.P[:, 0])
+    p_good = R1.T @ R1[:, 1]
+    p_bad = R1.T @ X[:, 1]
+    np.testing.assert_allclose(r.P[:, 1], p_good / np.linalg.norm(p_good), rtol=0, atol=1e-14)
+    assert np.max(np.abs(r.P[:, 1] - p_bad / np.linalg.norm(p_bad))) > 1e-3
+
+
+def test_separation_threshold_measurement(oracle_mod):
+    """DESIGN.md reading P9 (why single-vector parity is asserted only above a 2 % eigenvalue gap), as a measurement: the method
+    stops when lambda stagnates, so even the float64 oracle's loading vector is off the true singular vector
+    (LAPACK SVD) by about 0.15 eps / gap^2.  On the scaled config 3 (16 signal values with gaps of 0.5 ... 3.3 %), eps = 1e-7:
+    every component with a gap >= 2 % is within 5e-5 (half the north_star tolerance), components with 1 % <= gap < 1.5 % already
+    reach 1e-4 -- the tolerance itself -- so a 1 % separation rule would compare vectors that are not unique at that tolerance."""
+    cfg = inputs.scaled(inputs.config(2), 2048, 512, K=16)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    r = oracle_mod.pca(X, 17, 1e-7, 10000, oracle_mod.ALGO_GS, want_residual=False)
+    _, s, Vt = np.linalg.svd(X, full_matrices=False)
+    gap = np.array([min(abs(s[k] - s[j]) for j in range(17) if j != k) / s[k] for k in range(16)])
+    defect = np.array([1.0 - _abs_cos(r.P[:, k], Vt[k]) for k in range(16)])
+    assert np.all(defect[gap >= 0.02] <= 5e-5), (gap, defect)
+    assert np.all(defect <= 0.6e-7 / gap ** 2), (gap, defect)               # 1 - cos <~ 0.15 eps / gap^2, with a factor 4 of slack
+    narrow = (gap >= 0.01) & (gap < 0.015)
+    assert narrow.any() and defect[narrow].max() >= 1e-4, (gap, defect)

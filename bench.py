@@ -254,25 +254,74 @@ def e2e_leg(prob, X_np, steps):
     return dt, 4 * prob.M * prob.N, 4 * prob.K * (prob.M + prob.N) + 8 * prob.K
 
 
-def cpu_baseline_leg(cfg, algo, X_np, budget_s=20.0):
-    """The oracle as it stands, on this box's host cores, on a bounded sample of the workload:
-    the first components of the full-size problem (components are extracted one after the other,
-    so the first k_s components of the K-component solve ARE the k_s-component solve)."""
+# The bounded sample of each workload that BOTH oracle legs time (`cpu_baseline` of the CUDA arm and `--impl reference`):
+# the first k_s components of the full-size problem, solved to convergence.  Components are extracted one after the
+# other, so the first k_s components of the K-component solve ARE the k_s-component solve.
+ORACLE_SAMPLE_K = {"cfg1": 8, "cfg2": 32, "cfg3": 2, "cfg4": 8, "cfg5": 8}
+
+
+def oracle_sample(cfg, wname, algo, Xc, threads=None):
+    """Time the oracle as it stands on the sample; returns (k_s, seconds, inner iterations)."""
+    import oracle
+    ks = min(ORACLE_SAMPLE_K[wname], cfg.K)
+    n0 = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
+    try:
+        t0 = time.perf_counter()
+        r = oracle.pca(Xc, ks, cfg.eps, cfg.max_iter, algo, want_residual=False)
+        t = time.perf_counter() - t0
+    finally:
+        oracle.set_num_threads(n0)
+    return ks, t, int(r.iters.sum())
+
+
+def cpu_baseline_leg(cfg, wname, algo, X_np):
+    """The oracle as it stands, on this box's host cores, on the bounded sample of the workload (ORACLE_SAMPLE_K): all cores,
+    and -- on the first component only, to bound the time -- one thread."""
     import oracle
     Xc = oracle.center(X_np)
-    t0 = time.perf_counter()
-    r = oracle.pca(Xc, 1, cfg.eps, cfg.max_iter, algo, want_residual=False)
-    t1 = time.perf_counter() - t0
-    ks, t, its = 1, t1, int(r.iters.sum())
-    more = int(min(cfg.K, budget_s / max(t1, 1e-3)))
-    if more >= 2:                                               # cheap problem: a longer prefix
+    ks, t, its = oracle_sample(cfg, wname, algo, Xc)
+    cores = oracle.num_threads()
+    oracle.set_num_threads(1)
+    try:
         t0 = time.perf_counter()
-        r = oracle.pca(Xc, more, cfg.eps, cfg.max_iter, algo, want_residual=False)
-        t, ks, its = time.perf_counter() - t0, more, int(r.iters.sum())
-    return {"value": round(ks / t, 4), "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+        r1 = oracle.pca(Xc, 1, cfg.eps, cfg.max_iter, algo, want_residual=False)
+        t1 = time.perf_counter() - t0
+    finally:
+        oracle.set_num_threads(cores)
+    return {"value": round(ks / t, 4), "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"first {ks} of {cfg.K} components of {cfg.name} at full size ({its} inner iterations, "
-                      f"{t:.1f} s, float64, eps={cfg.eps:g})",
-            "us_per_inner_iteration": round(t / max(its, 1) * 1e6, 1)}
+                      f"{t:.1f} s, float64, eps={cfg.eps:g}); the same sample `--impl reference` times",
+            "us_per_inner_iteration": round(t / max(its, 1) * 1e6, 1),
+            "one_thread": {"value": round(1 / t1, 4), "unit": UNIT, "cores": 1,
+                           "sample": f"first component only ({int(r1.iters[0])} inner iterations, {t1:.1f} s)",
+                           "us_per_inner_iteration": round(t1 / max(int(r1.iters[0]), 1) * 1e6, 1)}}
+
+
+def validity_leg(prob):
+    """Sanity of the result of the LAST timed launch (outside the timed region; torch float64 on the device): the
+    exchange protocol's status word, orthogonality, ||T_k|| = lambda_k, and the energy identity of eq. (4)."""
+    torch, b = prob.torch, prob.binding
+    status = prob.ctx.pca_get_info(b.PCA_INFO_RUN_STATUS)
+    if status != 0:
+        raise SystemExit(f"bench.py: PCA_INFO_RUN_STATUS = {status}: an exchange wait gave up, the timed result is invalid")
+    K = prob.K
+    I = torch.eye(K, dtype=torch.float64, device="cuda")
+    Pd, Td, lam = prob.P.double(), prob.T.double(), prob.lam.double()
+    live = lam > 0
+    gp = float((Pd @ Pd.T - I)[live][:, live].abs().max())
+    tn = Td.norm(dim=1)
+    vd = Td / tn.clamp_min(1e-300)[:, None]
+    gv = float((vd @ vd.T - I)[live][:, live].abs().max())
+    tl = float(((tn - lam).abs() / lam.clamp_min(1e-300))[live].max())
+    x2 = float((prob.X.double() ** 2).sum())
+    r2 = float((prob.ctx.pca_residual().double() ** 2).sum())
+    return {"run_status": status, "max_abs_PtP_minus_I": gp, "max_abs_VtV_minus_I": gv if prob.gs() else None,
+            "max_rel_normT_minus_lambda": tl, "energy_identity_defect": abs(r2 - (x2 - float((lam ** 2).sum()))) / x2,
+            "degenerate_components": int((~live).sum()),
+            "note": "computed from the outputs of the last timed launch, after the timed region (float64 on the device); "
+                    "GS-PCA bound of the north_star: max|P^T P - I| <= 1e-5"}
 
 
 def pick_algo(cfg):
@@ -324,6 +373,9 @@ def run_cuda_arm(args):
     ms_per_step = step_ms / args.steps
     value = aggregate_value(K, world, ms_per_step)
     roof, iters = roofline(prob, run_ms, peaks)
+    validity = validity_leg(prob)
+    if prob.gs() and not args.fixed_iters and validity["max_abs_PtP_minus_I"] > 1e-5:
+        raise SystemExit(f"bench.py: the timed result is not orthogonal: {validity}")
 
     out = None
     if rank == 0:
@@ -344,6 +396,7 @@ def run_cuda_arm(args):
             "wall_s_timed_region": round(t_wall, 3),
             "clocks": clocks,
             "roofline": roof,
+            "validity": validity,
             "inner_iterations": {"total": int(iters.sum()), "max_per_component": int(iters.max()),
                                  "hit_max_iter": int((iters >= max_iter).sum()) if not args.fixed_iters else None},
         }
@@ -388,7 +441,7 @@ def run_cuda_arm(args):
             del pa
     # ---- cpu_baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline_leg(cfg, algo, pr.X, args.cpu_budget)
+        out["cpu_baseline"] = cpu_baseline_leg(cfg, args.workload, algo, pr.X)
     if rank == 0:
         print(json.dumps(out), flush=True)
     if world > 1:
@@ -409,16 +462,15 @@ def run_reference_arm(args):
     cfg = inputs.config(ci)
     algo = pick_algo(cfg)
     pr = inputs.generate(cfg)
-    ks = 1                                                      # bounded sample: the first component, full size
-    times, its = [], 0
+    times, its, ks = [], 0, 0
     for i in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         Xs = oracle.center(pr.X)                                # the step includes S0, like the CUDA arm's
-        r = oracle.pca(Xs, ks, cfg.eps, cfg.max_iter, algo, want_residual=False)
+        ks, _, n_it = oracle_sample(cfg, args.workload, algo, Xs)   # the same sample as the CUDA arm's cpu_baseline
         dt = time.perf_counter() - t0
         if i >= args.warmup:
             times.append(dt)
-            its = int(r.iters.sum())
+            its = n_it
     ms = float(np.mean(times)) * 1e3
     value = ks / (ms * 1e-3)
     sample = (f"each step = S0 centring + the first {ks} of {cfg.K} components of {cfg.name} at full size "
@@ -495,7 +547,6 @@ def main():
     ap.add_argument("--components", type=int, default=0, help="override K (profiling runs)")
     ap.add_argument("--fixed-iters", type=int, default=0, help="eps=0, max_iter=J: exactly J passes per component")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true")
     ap.add_argument("--also", default="all", help="other configs measured beside the workload: all | comma list of cfg1,cfg2,cfg3,cfg5")

@@ -50,7 +50,9 @@ enum {
   PCA_EALIGN = 2,       /* a device matrix pointer is not 16-byte aligned */
   PCA_ECUDA = 3,        /* a CUDA runtime call failed (pca_last_cuda_error has the code) */
   PCA_EWORKSPACE = 4,   /* no workspace set, or it is smaller than pca_workspace_bytes() */
-  PCA_EUNSUPPORTED = 5  /* shape cannot be handled by this build (e.g. N too large for SMEM) */
+  PCA_EUNSUPPORTED = 5, /* shape / option combination cannot be handled by this build (e.g. N too large for SMEM) */
+  PCA_EPROTOCOL = 6     /* pca_fit_host only: a cross-CTA exchange wait of the persistent kernel gave up (status word
+                           PCA_INFO_RUN_STATUS != 0); the results of that run are invalid.  Never in a correct run */
 };
 
 /* Options for pca_set_option (all optional; defaults are chosen by pca_create). */
@@ -66,8 +68,18 @@ enum {
                            levels for k > this value (-1 = default) */
   PCA_OPT_TEST_MODE = 7, /* convergence test: 0 = the listings' strict relative test |lambda - lambda'| < eps*lambda'
                            (default), 1 = the text's absolute test |lambda' - lambda| <= eps */
-  PCA_OPT_TRACE = 4     /* single-sweep kernels only: capacity (records) of the device-side phase trace, 0 = off
+  PCA_OPT_TRACE = 4,    /* single-sweep kernels only: capacity (records) of the device-side phase trace, 0 = off
                            (default).  See pca_trace. */
+  PCA_OPT_STAGNATION = 8, /* 1 (default): besides the listings' test, lambda' is also compared with the value TWO passes back
+                           (reading C4b: in fp32 the iteration can end in a period-2 limit cycle that the
+                           listings' test never sees); 0: the listings' / text's test alone, literally */
+  PCA_OPT_OUTPUT = 9,   /* 0 (default): PCA output, T = V Lambda, ||T[:,k]|| = lambda[k];
+                           1: SVD output "V, U, Lambda" (eq. 5 :56): T holds the UNIT score vectors V
+                           (the epilogue S10 is skipped; NIPALS-PCA: t / lambda), P = U, lambda = Lambda */
+  PCA_OPT_GS_PASSES = 10 /* GS-PCA: classical Gram-Schmidt projections per side per inner pass.  1 (default) = the listings
+                           (PAPER.md:1025-1026, :1030-1031); 2 = CGS2, "applying it iteratively".  2 is built
+                           into the two-sweep kernel only: the plan falls back to paths 1/2, forcing paths 3-6 gives
+                           PCA_EUNSUPPORTED.  Ignored for NIPALS-PCA */
 };
 
 /* Phase ids of the trace records (pca_trace).  One inner pass of the single-sweep kernel is
@@ -111,8 +123,10 @@ enum {
  *             component k is column k of the residual)
  *   eps       >= 0; relative stagnation tolerance of the listings' test
  *             |lambda - lambda'| < eps * lambda'; lambda' is also compared with
- *             the value two passes back (a period-2 limit cycle in fp32 is stagnation, C4b).  eps = 0 never fires,
- *             i.e. exactly max_iter passes per component (fixed-work benchmark mode)
+ *             the value two passes back (a period-2 limit cycle in fp32 is stagnation, C4b; PCA_OPT_STAGNATION = 0
+ *             switches that off).  With the default relative test eps = 0 never fires, i.e. exactly max_iter passes per
+ *             component (fixed-work benchmark mode); with PCA_OPT_TEST_MODE = 1 (|lambda' - lambda| <= eps) eps = 0 DOES
+ *             fire once lambda' repeats exactly, as the text's test says
  *   max_iter  >= 1; the listings' J = 10000
  *   algo      PCA_ALGO_NIPALS or PCA_ALGO_GS
  * Needs a CUDA device (queries its SM count and shared-memory size); PCA_ECUDA if there is none.
@@ -120,8 +134,9 @@ enum {
 int pca_create(pca_ctx** out, int64_t M, int64_t N, int K, double eps, int max_iter, int algo);
 
 /* Tune / query the launch plan.  pca_set_option must be called before pca_workspace_bytes /
- * pca_set_workspace; it re-plans and may return PCA_EUNSUPPORTED (e.g. forcing the resident path
- * for a matrix that does not fit in shared memory). */
+ * pca_set_workspace; it re-plans (a previously set workspace is dropped: set it again) and may return
+ * PCA_EUNSUPPORTED (e.g. forcing the resident path for a matrix that does not fit in shared memory),
+ * in which case the context keeps its previous options and plan. */
 int pca_set_option(pca_ctx*, int option, int64_t value);
 int pca_get_info(const pca_ctx*, int field, int64_t* value);
 
@@ -147,7 +162,8 @@ int pca_center(pca_ctx*, float* X, void* stream);
 /* The hot path: K components of NIPALS-PCA / GS-PCA on a centred X.
  *   X       dev, M x N, ld = M, centred; never written (R <- X)
  *   T       dev, M x K, ld = M, scores.  ||T[:,k]|| = lambda[k] for both algorithms
- *           (NIPALS: t = R p; GS-PCA: T = V Lambda)
+ *           (NIPALS: t = R p; GS-PCA: T = V Lambda); with
+ *           PCA_OPT_OUTPUT = 1 the unit vectors V instead (SVD output)
  *   P       dev, N x K, ld = N, loadings with unit columns
  *   lambda  dev, K floats, the last lambda' = ||T^(k)|| of each component (the paper's
  *           "eigenvalue" = singular value of the centred X); extraction order
@@ -179,8 +195,9 @@ int pca_trace(const pca_ctx*, const uint64_t** records, int64_t* capacity);
 /* Convenience entry with HOST buffers (used for end-to-end timing): copies X (host, M x N,
  * NOT centred) to the device, runs pca_center and pca_run on `stream`, copies T, P, lambda, iters
  * back and synchronises the stream.  The context allocates private device staging buffers and
- * the workspace on first use (freed by pca_destroy).  Host buffers should be pinned for full
- * PCIe bandwidth but need not be.  Errors: as pca_center / pca_run. */
+ * the workspace on first use (freed by pca_destroy; re-allocated if a later pca_set_option needs a
+ * larger one).  Host buffers should be pinned for full PCIe bandwidth but need not be.  After the
+ * synchronisation the run's status word is checked.  Errors: as pca_center / pca_run, PCA_EPROTOCOL. */
 int pca_fit_host(pca_ctx*, const float* X_host, float* T_host, float* P_host, float* lambda_host,
                  int32_t* iters_host, void* stream);
 

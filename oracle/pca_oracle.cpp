@@ -161,12 +161,16 @@ int oracle_center_eq1(double* X, int64_t M, int64_t N) {
 // returns 0, or 1 on invalid arguments.
 //   test_mode  0: the listings' strict relative test |lambda - lambda'| < eps*lambda' (reading C3, default)
 //              1: the text's / pseudo-code's absolute test |lambda' - lambda| <= eps
-int oracle_pca_ex(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo, int test_mode,
-                  double* T, double* P, double* lambda, int32_t* iters, double* R_out) {
+//   gs_passes  GS-PCA: classical Gram-Schmidt projections per side per inner pass.  1 = the listings (PAPER.md:1025-1026,
+//              :1030-1031; reading C9, default); 2 = "applying it iteratively" (CGS2): each projection is simply
+//              done twice in a row.  In exact arithmetic the second projection is the identity.
+int oracle_pca_ex2(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo, int test_mode,
+                   int gs_passes, double* T, double* P, double* lambda, int32_t* iters, double* R_out) {
   if (!X || !T || !P || !lambda || !iters) return 1;
   if (M < 1 || N < 1 || K < 1 || K > N || !(eps >= 0.0) || max_iter < 1) return 1;
   if (algo != 0 && algo != 1) return 1;
   if (test_mode != 0 && test_mode != 1) return 1;
+  if (gs_passes != 1 && gs_passes != 2) return 1;
   const bool gs = (algo == 1);
 
   std::vector<double> Rv((size_t)M * (size_t)N);
@@ -184,7 +188,7 @@ int oracle_pca_ex(const double* X, int64_t M, int64_t N, int K, double eps, int 
     bool degenerate = (nrm2(t, M) == 0.0);                           // reading C7
     for (int j = 0; j < max_iter && !degenerate; ++j) {              // PAPER.md:561,:1022 (C5)
       gemv_t(R, M, N, t, p);                                         // P^(k) <- R^T T^(k)
-      if (gs && k > 0) {
+      for (int rep = 0; gs && k > 0 && rep < gs_passes; ++rep) {
         gemv_t(P, N, k, p, coef.data());                             // A <- U_(k)^T U^(k)
         for (int i = 0; i < k; ++i) {                                // U^(k) <- U^(k) - U_(k) A
           const double a = coef[i];
@@ -196,7 +200,7 @@ int oracle_pca_ex(const double* X, int64_t M, int64_t N, int K, double eps, int 
       if (pn == 0.0) { degenerate = true; break; }                   // reading C7
       for (int64_t n = 0; n < N; ++n) p[n] /= pn;
       gemv_n(R, M, N, p, t);                                         // T^(k) <- R P^(k)
-      if (gs && k > 0) {
+      for (int rep = 0; gs && k > 0 && rep < gs_passes; ++rep) {
         gemv_t(T, M, k, t, coef.data());                             // B <- V_(k)^T V^(k)
         for (int i = 0; i < k; ++i) {                                // V^(k) <- V^(k) - V_(k) B
           const double b = coef[i];
@@ -230,6 +234,11 @@ int oracle_pca_ex(const double* X, int64_t M, int64_t N, int K, double eps, int 
       for (int64_t m = 0; m < M; ++m) T[id(m, k, M)] *= lambda[k];
   if (R_out) std::memcpy(R_out, R, sizeof(double) * (size_t)M * (size_t)N);
   return 0;
+}
+
+int oracle_pca_ex(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo, int test_mode,
+                  double* T, double* P, double* lambda, int32_t* iters, double* R_out) {
+  return oracle_pca_ex2(X, M, N, K, eps, max_iter, algo, test_mode, 1, T, P, lambda, iters, R_out);
 }
 
 int oracle_pca(const double* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo,

@@ -50,6 +50,7 @@ def _load():
         lib.oracle_center_eq1.argtypes = [dp, i64, i64]
         lib.oracle_pca.argtypes = [dp, i64, i64, i32, f64, i32, i32, dp, dp, dp, ip, dp]
         lib.oracle_pca_ex.argtypes = [dp, i64, i64, i32, f64, i32, i32, i32, dp, dp, dp, ip, dp]
+        lib.oracle_pca_ex2.argtypes = [dp, i64, i64, i32, f64, i32, i32, i32, i32, dp, dp, dp, ip, dp]
         lib.oracle_jacobi_eigh.argtypes = [dp, i32, dp, dp, i32, f64]
         _lib = lib
     return _lib
@@ -102,9 +103,10 @@ class OracleResult:
 
 
 def pca(X, K: int, eps: float = 1e-7, max_iter: int = 10000, algo: int = ALGO_GS,
-        want_residual: bool = True, test_mode: int = 0) -> OracleResult:
+        want_residual: bool = True, test_mode: int = 0, gs_passes: int = 1) -> OracleResult:
     """Run the oracle's NIPALS-PCA / GS-PCA on an (already centred) M x N matrix.
-    test_mode 0: the listings' strict relative test; 1: the text's absolute test."""
+    test_mode 0: the listings' strict relative test; 1: the text's absolute test.
+    gs_passes 1: one classical Gram-Schmidt projection per side per pass (the listings); 2: CGS2."""
     Xd = _as_f64_colmajor(X)
     M, N = Xd.shape
     T = np.zeros((M, K), dtype=np.float64, order="F")
@@ -112,7 +114,7 @@ def pca(X, K: int, eps: float = 1e-7, max_iter: int = 10000, algo: int = ALGO_GS
     lam = np.zeros(K, dtype=np.float64)
     iters = np.zeros(K, dtype=np.int32)
     R = np.zeros((M, N), dtype=np.float64, order="F") if want_residual else None
-    rc = _load().oracle_pca_ex(_dptr(Xd), M, N, int(K), float(eps), int(max_iter), int(algo), int(test_mode),
+    rc = _load().oracle_pca_ex2(_dptr(Xd), M, N, int(K), float(eps), int(max_iter), int(algo), int(test_mode), int(gs_passes),
                                _dptr(T), _dptr(P), _dptr(lam),
                             iters.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
                             _dptr(R) if R is not None else None)

@@ -16,9 +16,10 @@ import os
 PCA_ALGO_NIPALS = 0
 PCA_ALGO_GS = 1
 
-PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED = range(6)
+PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED, PCA_EPROTOCOL = range(7)
 
 PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT, PCA_OPT_TEST_MODE = 1, 2, 3, 4, 5, 6, 7
+PCA_OPT_STAGNATION, PCA_OPT_OUTPUT, PCA_OPT_GS_PASSES = 8, 9, 10
 (PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT,
  PCA_PATH_REGISTER, PCA_PATH_ONE_CTA) = 0, 1, 2, 3, 4, 5, 6
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
@@ -259,6 +260,8 @@ def fit(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, path=P
     iters = torch.empty(K, dtype=torch.int32, device="cuda")
     ctx.pca_run(X, T, P, lam, iters)
     torch.cuda.synchronize()
+    if ctx.pca_get_info(PCA_INFO_RUN_STATUS) != 0:
+        raise PcaError(PCA_EPROTOCOL, "pca_run", "a cross-CTA exchange wait gave up (PCA_INFO_RUN_STATUS != 0)")
     out = dict(T=to_colmajor(T), P=to_colmajor(P), lam=lam.cpu().numpy(), iters=iters.cpu().numpy(),
                Xc=to_colmajor(X), info=ctx.info())
     if want_residual:

@@ -85,6 +85,7 @@ struct pca_ctx {
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
+  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -113,6 +114,7 @@ struct pca_ctx {
   float *hX = nullptr, *hT = nullptr, *hP = nullptr, *hLam = nullptr;
   int* hIters = nullptr;
   void* hWs = nullptr;
+  size_t hWs_bytes = 0;
   int last_cuda = 0;
 };
 
@@ -184,6 +186,9 @@ int make_fused_plan(pca_ctx* c, int want) {
   int GT = 32;
   while ((long long)16 * GT < N) GT *= 2;
   if (GT > pca::kThreads) return PCA_EUNSUPPORTED;
+  // the k-vectors A and B are combined with one thread per pair of entries (RegGather): at most kThreads pairs.
+  // Larger K with GS-PCA goes to the two-sweep kernel, whose coefficient reduction is chunked.
+  if (c->algo == PCA_ALGO_GS && (c->K + 1) / 2 + 1 > pca::kThreads) return PCA_EUNSUPPORTED;
   const int NV = (int)ceil_div(N, 4LL * GT);
   const int ldr = 4 * GT * NV;
   const int g_min = (int)ceil_div(N, pca::kThreads);
@@ -271,7 +276,7 @@ int make_fused_plan(pca_ctx* c, int want) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
   take((size_t)M * (size_t)N * 4);                                   // residual of eq. (4), column-major (ABI layout)
@@ -310,6 +315,7 @@ int make_reg_plan(pca_ctx* c) {
   int GT = 8;
   while (8LL * GT < N) GT *= 2;
   if (GT > pca::kThreads) return PCA_EUNSUPPORTED;
+  if (c->algo == PCA_ALGO_GS && (c->K + 1) / 2 + 1 > pca::kThreads) return PCA_EUNSUPPORTED;   // as make_fused_plan
   const int NG = pca::kThreads / GT, ldr = 8 * GT;
   int G = c->opt_ctas > 0 ? c->opt_ctas : (int)ceil_div(M, (long long)NG * 7);
   if (G < 1) G = 1;
@@ -372,7 +378,7 @@ int make_reg_plan(pca_ctx* c) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output;
   p.kdirect = c->opt_kdirect >= 0 ? (c->opt_kdirect > 30 ? 30 : c->opt_kdirect) : 0;    // direct: <= 16 units, one per warp
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
@@ -416,7 +422,7 @@ int make_one_plan(pca_ctx* c) {
   pca::one_kernel_t fn = pca::one_kernel_lookup(GT, RPT);
   if (!fn) return PCA_EUNSUPPORTED;
   OneParams p{};
-  p.M = (int)M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
+  p.M = (int)M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output;
   p.ldr = ldr; p.Kpad = (int)round_up(c->K, 4);
   const bool gs = c->algo == PCA_ALGO_GS;
   size_t off = 0;
@@ -459,17 +465,22 @@ int make_one_plan(pca_ctx* c) {
 
 int make_plan(pca_ctx* c) {
   c->planned = false;
-  if ((c->opt_path == 0 && c->opt_trace == 0) || c->opt_path == 6) {
+  // CGS2 (PCA_OPT_GS_PASSES = 2) is built into the two-sweep kernel only (paths 1, 2), whose pass has a separate phase
+  // per projection; the single-sweep kernels fold the scores-side projection into the loads by linearity and have no
+  // place for a second one.
+  const bool cgs2 = c->opt_gs_passes > 1 && c->algo == PCA_ALGO_GS;
+  if (cgs2 && c->opt_path >= 3) return PCA_EUNSUPPORTED;
+  if (!cgs2 && ((c->opt_path == 0 && c->opt_trace == 0) || c->opt_path == 6)) {
     const int rc = make_one_plan(c);
     if (rc == PCA_OK || c->opt_path != 0) return rc;
     if (rc == PCA_ECUDA) return rc;
   }
-  if (c->opt_path == 0 || c->opt_path == 5) {
+  if (!cgs2 && (c->opt_path == 0 || c->opt_path == 5)) {
     const int rc = make_reg_plan(c);
     if (rc == PCA_OK || c->opt_path != 0) return rc;
     if (rc == PCA_ECUDA) return rc;
   }
-  if (c->opt_path == 0 || c->opt_path == 3 || c->opt_path == 4) {
+  if (!cgs2 && (c->opt_path == 0 || c->opt_path == 3 || c->opt_path == 4)) {
     const int rc = make_fused_plan(c, c->opt_path);
     if (rc == PCA_OK || c->opt_path != 0) return rc;
     if (rc == PCA_ECUDA) return rc;
@@ -520,14 +531,15 @@ int make_plan(pca_ctx* c) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
+  p.M = M; p.N = N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output;
+  p.gs_passes = c->opt_gs_passes;
   // workspace layout: R first
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
   take((size_t)M * (size_t)N * 4);
   c->ws_off_ppart = take((size_t)p.G * p.Npad * 4);
-  c->ws_off_apart = take((size_t)p.Gs * p.Kpad * 8);
-  c->ws_off_bpart = take((size_t)p.G * p.Kpad * 8);
+  c->ws_off_apart = take((size_t)2 * p.Gs * p.Kpad * 8);            // one buffer per Gram-Schmidt projection (CGS2: two)
+  c->ws_off_bpart = take((size_t)2 * p.G * p.Kpad * 8);
   c->ws_off_pvec = take((size_t)p.Npad * 4);
   c->ws_off_qpart = take((size_t)p.Gs * 8);
   c->ws_off_spart = take((size_t)p.G * 8);
@@ -543,6 +555,55 @@ int make_plan(pca_ctx* c) {
   c->ran = false;
   return PCA_OK;
 }
+
+int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
+  switch (option) {
+    case PCA_OPT_PATH:
+      if (value < 0 || value > 6) return PCA_EINVAL;
+      c->opt_path = (int)value;
+      break;
+    case PCA_OPT_CTAS:
+      if (value < 0 || value > c->num_sms) return PCA_EINVAL;
+      c->opt_ctas = (int)value;
+      break;
+    case PCA_OPT_CENTER_MODE:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_center_mode = (int)value;
+      return PCA_OK;
+    case PCA_OPT_OWNERS:
+      if (value < 0 || value > c->num_sms) return PCA_EINVAL;
+      c->opt_owners = (int)value;
+      break;
+    case PCA_OPT_KDIRECT:
+      if (value < -1 || value > (1 << 30)) return PCA_EINVAL;
+      c->opt_kdirect = (int)value;
+      break;
+    case PCA_OPT_TEST_MODE:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_test_mode = (int)value;
+      break;
+    case PCA_OPT_TRACE:
+      if (value < 0 || value > (1 << 24)) return PCA_EINVAL;
+      c->opt_trace = (int)value;
+      break;
+    case PCA_OPT_STAGNATION:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_stag2 = (int)value;
+      break;
+    case PCA_OPT_OUTPUT:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_output = (int)value;
+      break;
+    case PCA_OPT_GS_PASSES:
+      if (value < 1 || value > 2) return PCA_EINVAL;
+      c->opt_gs_passes = (int)value;
+      break;
+    default:
+      return PCA_EINVAL;
+  }
+  return make_plan(c);
+}
+
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -579,39 +640,10 @@ int pca_create(pca_ctx** out, int64_t M, int64_t N, int K, double eps, int max_i
 
 int pca_set_option(pca_ctx* c, int option, int64_t value) {
   if (!c) return PCA_EINVAL;
-  switch (option) {
-    case PCA_OPT_PATH:
-      if (value < 0 || value > 6) return PCA_EINVAL;
-      c->opt_path = (int)value;
-      break;
-    case PCA_OPT_CTAS:
-      if (value < 0 || value > c->num_sms) return PCA_EINVAL;
-      c->opt_ctas = (int)value;
-      break;
-    case PCA_OPT_CENTER_MODE:
-      if (value < 0 || value > 1) return PCA_EINVAL;
-      c->opt_center_mode = (int)value;
-      return PCA_OK;
-    case PCA_OPT_OWNERS:
-      if (value < 0 || value > c->num_sms) return PCA_EINVAL;
-      c->opt_owners = (int)value;
-      break;
-    case PCA_OPT_KDIRECT:
-      if (value < -1 || value > (1 << 30)) return PCA_EINVAL;
-      c->opt_kdirect = (int)value;
-      break;
-    case PCA_OPT_TEST_MODE:
-      if (value < 0 || value > 1) return PCA_EINVAL;
-      c->opt_test_mode = (int)value;
-      break;
-    case PCA_OPT_TRACE:
-      if (value < 0 || value > (1 << 24)) return PCA_EINVAL;
-      c->opt_trace = (int)value;
-      break;
-    default:
-      return PCA_EINVAL;
-  }
-  return make_plan(c);
+  const pca_ctx saved = *c;                                      // a re-plan that fails leaves the context as it was
+  const int rc = pca_set_option_impl(c, option, value);
+  if (rc != PCA_OK) *c = saved;
+  return rc;
 }
 
 int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
@@ -742,7 +774,8 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     const dim3 ogrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(c->N, 32));
     pca::pca_transpose_out_kernel<<<ogrid, 256, 0, st>>>(p.Rrm, reinterpret_cast<float*>(ws),
                                                          T + (size_t)(c->K - 1) * (size_t)c->M,
-                                                         P + (size_t)(c->K - 1) * (size_t)c->N, c->M, p.N, p.ldr);
+                                                         P + (size_t)(c->K - 1) * (size_t)c->N,
+                                                         c->opt_output ? lambda + (c->K - 1) : nullptr, c->M, p.N, p.ldr);
     PCA_CUDA(c, cudaGetLastError());
     c->ran = true;
     return PCA_OK;
@@ -787,17 +820,27 @@ int pca_fit_host(pca_ctx* c, const float* X_host, float* T_host, float* P_host, 
   if (!c || !X_host || !T_host || !P_host || !lambda_host || !iters_host || !c->planned) return PCA_EINVAL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const size_t xb = (size_t)c->M * (size_t)c->N * 4, tb = (size_t)c->M * c->K * 4, pb = (size_t)c->N * c->K * 4;
-  if (!c->hX) {
-    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hX), xb));
-    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hT), tb));
-    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hP), pb));
-    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hLam), (size_t)c->K * 4));
-    PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hIters), (size_t)c->K * 4));
-  }
-  if (!c->ws) {
-    if (!c->hWs) PCA_CUDA(c, cudaMalloc(&c->hWs, c->ws_bytes));
+  // staging buffers (shape-dependent only; one pointer at a time so that a failed allocation is retried, not skipped)
+  if (!c->hX) PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hX), xb));
+  if (!c->hT) PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hT), tb));
+  if (!c->hP) PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hP), pb));
+  if (!c->hLam) PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hLam), (size_t)c->K * 4));
+  if (!c->hIters) PCA_CUDA(c, cudaMalloc(reinterpret_cast<void**>(&c->hIters), (size_t)c->K * 4));
+  if (!c->ws || c->ws == c->hWs) {
+    // private workspace: a re-plan (pca_set_option) may have grown pca_workspace_bytes() since it was allocated
+    if (c->hWs && c->hWs_bytes < c->ws_bytes) {
+      PCA_CUDA(c, cudaStreamSynchronize(st));
+      cudaFree(c->hWs);
+      c->hWs = nullptr;
+      c->hWs_bytes = 0;
+      c->ws = nullptr;
+    }
+    if (!c->hWs) {
+      PCA_CUDA(c, cudaMalloc(&c->hWs, c->ws_bytes));
+      c->hWs_bytes = c->ws_bytes;
+    }
     c->ws = c->hWs;
-    c->ws_given = c->ws_bytes;
+    c->ws_given = c->hWs_bytes;
   }
   PCA_CUDA(c, cudaMemcpyAsync(c->hX, X_host, xb, cudaMemcpyHostToDevice, st));
   int rc = pca_center(c, c->hX, stream);
@@ -808,7 +851,13 @@ int pca_fit_host(pca_ctx* c, const float* X_host, float* T_host, float* P_host, 
   PCA_CUDA(c, cudaMemcpyAsync(P_host, c->hP, pb, cudaMemcpyDeviceToHost, st));
   PCA_CUDA(c, cudaMemcpyAsync(lambda_host, c->hLam, (size_t)c->K * 4, cudaMemcpyDeviceToHost, st));
   PCA_CUDA(c, cudaMemcpyAsync(iters_host, c->hIters, (size_t)c->K * 4, cudaMemcpyDeviceToHost, st));
+  unsigned run_status = 0;                                       // the exchange protocol's status word (paths 3-5)
+  const bool has_status = c->path >= 3 && c->path != 6;
+  if (has_status)
+    PCA_CUDA(c, cudaMemcpyAsync(&run_status, static_cast<const unsigned char*>(c->ws) + c->ws_off_status, sizeof(run_status),
+                                cudaMemcpyDeviceToHost, st));
   PCA_CUDA(c, cudaStreamSynchronize(st));
+  if (has_status && run_status != 0) return PCA_EPROTOCOL;
   return PCA_OK;
 }
 
@@ -831,6 +880,7 @@ const char* pca_strerror(int code) {
     case PCA_ECUDA: return "CUDA runtime error (no device, or a launch/copy failed)";
     case PCA_EWORKSPACE: return "workspace missing or too small";
     case PCA_EUNSUPPORTED: return "shape not supported by this build";
+    case PCA_EPROTOCOL: return "a cross-CTA exchange wait gave up: the results of this run are invalid";
     default: return "unknown error";
   }
 }

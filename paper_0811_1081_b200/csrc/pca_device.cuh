@@ -91,10 +91,12 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 // mode 0: the listings' strict relative test |lambda - lambda'| < eps*lambda' (reading C3, default)
 // mode 1: the text's / pseudo-code's absolute test |lambda' - lambda| <= eps
 // lam = lambda of the previous pass (0 before the first), lam2 = of the one before (0 = none yet):
-// reading C4b, a period-2 limit cycle of lambda' in fp32 is stagnation too.
-__device__ __forceinline__ bool pca_stagnated(double lam, double lam2, double ln, double eps, int mode) {
-  if (mode == 1) return fabs(ln - lam) <= eps || (lam2 > 0.0 && fabs(ln - lam2) <= eps);
-  return fabs(lam - ln) < eps * ln || (lam2 > 0.0 && fabs(lam2 - ln) < eps * ln);
+// reading C4b (stag2 != 0, PCA_OPT_STAGNATION = 1, the default): a period-2 limit cycle of lambda' in fp32 is stagnation
+// too, so lambda' is also compared with the value two passes back.  stag2 == 0: the listing's / text's test alone.
+__device__ __forceinline__ bool pca_stagnated(double lam, double lam2, double ln, double eps, int mode, int stag2) {
+  const bool two = stag2 != 0 && lam2 > 0.0;
+  if (mode == 1) return fabs(ln - lam) <= eps || (two && fabs(ln - lam2) <= eps);
+  return fabs(lam - ln) < eps * ln || (two && fabs(lam2 - ln) < eps * ln);
 }
 
 // ------------------------------------------------------------------------------------ block reductions

@@ -53,6 +53,8 @@ struct FusedParams {
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
   int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
+  int stag2;             // reading C4b: also compare lambda' with the value two passes back (PCA_OPT_STAGNATION)
+  int out_svd;           // PCA_OPT_OUTPUT = 1: T holds the unit score vectors V (SVD triple V, U = P, Lambda)
   int G;                 // CTAs
   int Mb;                // rows per CTA
   int ldr;               // row stride of Rrm / slab (floats) = 4*GT*NV
@@ -655,7 +657,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
             ln = sqrt(l2);                                                    // S7
             // S8: listings' strict relative test (reading C3)
             // (+ reading C4b: a period-2 limit cycle of lambda' in fp32 is stagnation too)
-            if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode) || (it >= prm.max_iter)) st = 1;
+            if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode, prm.stag2) || (it >= prm.max_iter)) st = 1;
           }
         }
         if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }
@@ -847,7 +849,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           t -= corr;
         }
         d_s[i] = t;                                                           // R -= lambda v p^T  /  R -= t p^T
-        Tb[(size_t)k * M + i] = gs ? t * inv : t;
+        Tb[(size_t)k * M + i] = (gs || prm.out_svd) ? t * inv : t;
         if (gs && k < prm.Ksm) Vc[(size_t)k * prm.Mbp + i] = t * inv;
       }
       if (tid < ns) {
@@ -868,8 +870,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
 
   // resident: hand the slab back (the last deflation is applied by pca_transpose_out_kernel)
   if constexpr (RESIDENT) sweep_loads<NV, SRC_SLAB, DST_GLOBAL, false, false>(prm, Rb, slab, mb, ttil_s, d_s, pdef_s, qs);
-  // ---- S10: GS-PCA  T <- V Lambda ----
-  if (gs) {
+  // ---- S10: GS-PCA  T <- V Lambda; skipped for the SVD output V, U, Lambda ----
+  if (gs && !prm.out_svd) {
     __syncthreads();
     for (int kk = 0; kk < K; ++kk) {
       const float l = lam_s[kk];
@@ -903,19 +905,21 @@ static __global__ void __launch_bounds__(256) pca_transpose_in_kernel(const floa
 
 // Rout[n*M + m] = Rrm[m][n] - d[m]*p[n]: the residual of eq. (4) in the ABI's column-major layout,
 // with the last component's deflation (d = T[:,K-1] after the epilogue, p = P[:,K-1]) applied.
+// dscale != nullptr (SVD output: T holds unit vectors): d is scaled by dscale[0] = lambda[K-1].
 static __global__ void __launch_bounds__(256) pca_transpose_out_kernel(const float* __restrict__ Rrm, float* __restrict__ Rout,
                                                                 const float* __restrict__ d, const float* __restrict__ p,
-                                                                long long M, int N, int ldr) {
+                                                                const float* __restrict__ dscale, long long M, int N, int ldr) {
   __shared__ float tile[32][33];
   const long long mt = (long long)blockIdx.x * 32;
   const int nt = blockIdx.y * 32;
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const float ds = dscale ? __ldcg(dscale) : 1.f;
 #pragma unroll
   for (int j = ty; j < 32; j += 8) {
     const long long m = mt + j;
     const int n = nt + tx;
     float v = 0.f;
-    if (m < M && n < N) v = fmaf(-__ldcg(d + m), __ldcg(p + n), __ldcg(Rrm + (size_t)m * ldr + n));
+    if (m < M && n < N) v = fmaf(-__ldcg(d + m) * ds, __ldcg(p + n), __ldcg(Rrm + (size_t)m * ldr + n));
     tile[j][tx] = v;
   }
   __syncthreads();

@@ -25,6 +25,8 @@ struct OneParams {
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
   int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
+  int stag2;             // reading C4b: also compare lambda' with the value two passes back (PCA_OPT_STAGNATION)
+  int out_svd;           // PCA_OPT_OUTPUT = 1: T holds the unit score vectors V (SVD triple V, U = P, Lambda)
   int ldr;               // 8*GT >= N
   int Kpad;
   // shared-memory carve-up (byte offsets)
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
           else {
             ln = sqrt(l2);                                                    // S7
             // S8: the listings' strict relative test (readings C3, C4b)
-            if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode) || (it >= prm.max_iter)) st = 1;
+            if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode, prm.stag2) || (it >= prm.max_iter)) st = 1;
           }
         }
         if (lane == 0) { ctl_s[1] = ln; reinterpret_cast<int*>(ctl_s + 2)[0] = st; }
@@ -213,7 +215,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
       one_rowdot(Vb, KV, B_s, mb, gsk ? k : 0, one_parts(mb), [&](int r, double a) {
         const float t = ttil_s[r] - (float)a;
         d_s[r] = t;
-        prm.T[(size_t)k * M + r] = t;
+        prm.T[(size_t)k * M + r] = prm.out_svd ? t * inv : t;                 // SVD output: the unit vector v
         if (gs) Vb[(size_t)r * KV + k] = t * inv;
       });
       for (int c = tid; c < ldr; c += kThreads) {

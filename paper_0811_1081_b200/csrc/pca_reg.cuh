@@ -39,6 +39,8 @@ struct RegParams {
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
   int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
+  int stag2;             // reading C4b: also compare lambda' with the value two passes back (PCA_OPT_STAGNATION)
+  int out_svd;           // PCA_OPT_OUTPUT = 1: T holds the unit score vectors V (SVD triple V, U = P, Lambda)
   int G;                 // CTAs
   int Mb;                // rows per CTA (<= NG*RPT)
   int ldr;               // 4*NV*GT >= N
@@ -577,7 +579,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
               // S8: the listings' strict relative test (reading C3)
               // (+ reading C4b: in fp32 the iteration can end in a period-2 limit cycle, lambda' alternating between two
               //  values; that is stagnation too, so lambda' is also compared with the value two passes back)
-              if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode) || (it >= prm.max_iter)) st = 1;
+              if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode, prm.stag2) || (it >= prm.max_iter)) st = 1;
             }
           }
           if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }
@@ -758,7 +760,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         if (lane == 0) {
           const float t = ttil_s[r] - corr;
           d_s[r] = t;                                                         // S9: R -= lambda' v p^T  /  R -= t p^T
-          Tb[(size_t)k * M + r] = t;
+          Tb[(size_t)k * M + r] = prm.out_svd ? t * inv : t;                  // SVD output: the unit vector v
           if (gs) Vb[(size_t)r * KV + k] = t * inv;
         }
       }

@@ -38,6 +38,10 @@ struct SolveParams {
   int max_iter;
   int algo;              // 0 NIPALS, 1 GS
   int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
+  int stag2;             // reading C4b: also compare lambda' with the value two passes back (PCA_OPT_STAGNATION)
+  int out_svd;           // PCA_OPT_OUTPUT = 1: T holds the unit score vectors V (SVD triple V, U = P, Lambda)
+  int gs_passes;         // classical Gram-Schmidt projections per side per inner pass: 1 (the listings), 2 = CGS2 ("applying it
+                         // iteratively"; PCA_OPT_GS_PASSES)
   int G;                 // CTAs
   int Mb;                // rows per CTA (uniform; last CTAs may own fewer / none)
   int Ns;                // columns per slice owner (multiple of 4)
@@ -46,8 +50,8 @@ struct SolveParams {
   int Npad;              // row stride of Ppart (floats)
   int Kpad;              // row stride of Apart / Bpart (doubles)
   float* Ppart;          // [G][Npad]   partial loads
-  double* Apart;         // [Gs][Kpad]  partial A (loads-side GS coefficients)
-  double* Bpart;         // [G][Kpad]   partial B (scores-side GS coefficients)
+  double* Apart;         // [2][Gs][Kpad]  partial A (loads-side GS coefficients), one buffer per CGS projection
+  double* Bpart;         // [2][G][Kpad]   partial B (scores-side GS coefficients)
   float* pvec;           // [Npad]      p^ (orthogonalised, not yet normalised)
   double* qpart;         // [Gs]        ||p^||^2 partials
   double* spart;         // [G]         ||t||^2 partials
@@ -137,33 +141,36 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
         __syncthreads();
       }
       if (gs && k > 0) {
-        // ---- S3: A-partials  a_b[jj] = sum_{n in slice} P[n,jj] p~[n] ----
-        if (ns > 0) {
-          for (int jj = tid; jj < k; jj += kThreads) {
-            const float* pj = prm.P + (size_t)jj * N + n0;
-            double a = 0.0;
-            for (int i = 0; i < ns; ++i) a += (double)ld_cg(pj + i) * (double)slice_s[i];
-            prm.Apart[(size_t)b * prm.Kpad + jj] = a;
+        for (int rep = 0; rep < prm.gs_passes; ++rep) {                  // CGS2: project a second time
+          double* Apart = prm.Apart + (size_t)rep * prm.Gs * prm.Kpad;
+          // ---- S3: A-partials  a_b[jj] = sum_{n in slice} P[n,jj] p~[n] ----
+          if (ns > 0) {
+            for (int jj = tid; jj < k; jj += kThreads) {
+              const float* pj = prm.P + (size_t)jj * N + n0;
+              double a = 0.0;
+              for (int i = 0; i < ns; ++i) a += (double)ld_cg(pj + i) * (double)slice_s[i];
+              Apart[(size_t)b * prm.Kpad + jj] = a;
+            }
           }
-        }
-        grid_barrier(prm.bar, bar_target, G);
-        // ---- Ph3: A = sum of partials;  p^ = p~ - P_(k) A ----
-        if (ns > 0) {
-          reduce_coef_parts(coef_s, prm.Apart, k, prm.Gs, prm.Kpad, scr);
-          const int nsub = kThreads / ns;
-          const int sub = tid / ns, i = tid - sub * ns;
-          double v = 0.0;
-          if (sub < nsub)
-            for (int jj = sub; jj < k; jj += nsub) v += (double)ld_cg(prm.P + (size_t)jj * N + n0 + i) * coef_s[jj];
-          __syncthreads();
-          if (sub < nsub) scr[sub * ns + i] = v;
-          __syncthreads();
-          if (tid < ns) {
-            double s = 0.0;
-            for (int q = 0; q < nsub; ++q) s += scr[q * ns + tid];
-            slice_s[tid] = (float)((double)slice_s[tid] - s);
+          grid_barrier(prm.bar, bar_target, G);
+          // ---- Ph3: A = sum of partials;  p^ = p~ - P_(k) A ----
+          if (ns > 0) {
+            reduce_coef_parts(coef_s, Apart, k, prm.Gs, prm.Kpad, scr);
+            const int nsub = kThreads / ns;
+            const int sub = tid / ns, i = tid - sub * ns;
+            double v = 0.0;
+            if (sub < nsub)
+              for (int jj = sub; jj < k; jj += nsub) v += (double)ld_cg(prm.P + (size_t)jj * N + n0 + i) * coef_s[jj];
+            __syncthreads();
+            if (sub < nsub) scr[sub * ns + i] = v;
+            __syncthreads();
+            if (tid < ns) {
+              double s = 0.0;
+              for (int q = 0; q < nsub; ++q) s += scr[q * ns + tid];
+              slice_s[tid] = (float)((double)slice_s[tid] - s);
+            }
+            __syncthreads();
           }
-          __syncthreads();
         }
       }
       // ---- S4 (first half): ||p^||^2 partial, publish the slice ----
@@ -189,23 +196,26 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       else                    pass_n<VEC, TR, RC, SRC_GLOBAL>(Rb, M, nullptr, 0, mb, N, p_s, t_s, red_s);
 
       if (gs && k > 0) {
-        // ---- S6: B-partials  b_b[jj] = sum_{rows} V[m,jj] t[m] ----
-        for (int jj = w; jj < k; jj += kWarps) {
-          const float* vj = Tb + (size_t)jj * M;
-          float a = 0.f;
-          for (int i = lane; i < mb; i += 32) a = fmaf(ld_cg(vj + i), t_s[i], a);
-          const double s = warp_sum((double)a);
-          if (lane == 0) prm.Bpart[(size_t)b * prm.Kpad + jj] = s;
+        for (int rep = 0; rep < prm.gs_passes; ++rep) {                  // CGS2: project a second time
+          double* Bpart = prm.Bpart + (size_t)rep * G * prm.Kpad;
+          // ---- S6: B-partials  b_b[jj] = sum_{rows} V[m,jj] t[m] ----
+          for (int jj = w; jj < k; jj += kWarps) {
+            const float* vj = Tb + (size_t)jj * M;
+            float a = 0.f;
+            for (int i = lane; i < mb; i += 32) a = fmaf(ld_cg(vj + i), t_s[i], a);
+            const double s = warp_sum((double)a);
+            if (lane == 0) Bpart[(size_t)b * prm.Kpad + jj] = s;
+          }
+          grid_barrier(prm.bar, bar_target, G);
+          // ---- Ph5: B = sum of partials;  t -= V_(k) B ----
+          reduce_coef_parts(coef_s, Bpart, k, G, prm.Kpad, scr);
+          for (int i = tid; i < mb; i += kThreads) {
+            float corr = 0.f;
+            for (int jj = 0; jj < k; ++jj) corr = fmaf(ld_cg(Tb + (size_t)jj * M + i), (float)coef_s[jj], corr);
+            t_s[i] -= corr;
+          }
+          __syncthreads();
         }
-        grid_barrier(prm.bar, bar_target, G);
-        // ---- Ph5: B = sum of partials;  t -= V_(k) B ----
-        reduce_coef_parts(coef_s, prm.Bpart, k, G, prm.Kpad, scr);
-        for (int i = tid; i < mb; i += kThreads) {
-          float corr = 0.f;
-          for (int jj = 0; jj < k; ++jj) corr = fmaf(ld_cg(Tb + (size_t)jj * M + i), (float)coef_s[jj], corr);
-          t_s[i] -= corr;
-        }
-        __syncthreads();
       }
       // ---- S7: lambda' = ||t|| ----
       {
@@ -225,7 +235,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       }
       it = j + 1;
       // ---- S8: listings' strict relative test (reading C3) ----
-      if (pca_stagnated(lam, lam2, lam_new, prm.eps, prm.test_mode)) break;   // S8 (readings C3, C4b)
+      if (pca_stagnated(lam, lam2, lam_new, prm.eps, prm.test_mode, prm.stag2)) break;   // S8 (readings C3, C4b)
       lam2 = lam;
       lam = lam_new;
     }
@@ -238,9 +248,10 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       if (tid == 0) lam_s[k] = 0.f;
     } else {
       const float lamf = (float)lam_new;
+      const float tscale = (!gs && prm.out_svd) ? (float)(1.0 / lam_new) : 1.f;   // SVD output of NIPALS-PCA: v = t/lambda
       for (int i = tid; i < mb; i += kThreads) {
         const float v = t_s[i];
-        Tb[(size_t)k * M + i] = v;                                    // GS-PCA: unit v until the final scaling
+        Tb[(size_t)k * M + i] = v * tscale;                           // GS-PCA: unit v until the final scaling
         d_s[i] = gs ? lamf * v : v;                                   // R -= lambda v p^T / R -= t p^T
       }
       if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = p_s[n0 + tid];
@@ -255,8 +266,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
     pass_t<VEC, TR, RC, SRC_SLAB, DST_GLOBAL, true, false>(nullptr, Rb, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
   else
     pass_t<VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, false>(Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
-  // ---- S10: GS-PCA  T <- V Lambda ----
-  if (gs) {
+  // ---- S10: GS-PCA  T <- V Lambda; skipped for the SVD output V, U, Lambda ----
+  if (gs && !prm.out_svd) {
     __syncthreads();
     for (int kk = 0; kk < K; ++kk) {
       const float l = lam_s[kk];

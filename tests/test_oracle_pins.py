@@ -390,3 +390,27 @@ def test_separation_threshold_measurement(oracle_mod):
     assert np.all(defect <= 0.6e-7 / gap ** 2), (gap, defect)               # 1 - cos <~ 0.15 eps / gap^2, with a factor 4 of slack
     narrow = (gap >= 0.01) & (gap < 0.015)
     assert narrow.any() and defect[narrow].max() >= 1e-4, (gap, defect)
+
+
+def test_cgs2_mode_is_the_identity_in_double(oracle_mod):
+    """gs_passes = 2 (CGS2, "applying it iteratively"): in exact arithmetic the second projection removes
+    nothing, so in float64 the results agree with the listings' single projection to rounding and orthogonality is not
+    worse -- for converged runs and for early-stopped ones (max_iter = 1), where the first projection is doing real work.
+    (The second projection itself is visible only at the rounding level: this idempotence is its pin.)"""
+    cfg = inputs.scaled(inputs.config(2), 300, 80, K=12)
+    X = oracle_mod.center(inputs.generate(cfg).X)
+    for max_iter in (10000, 1):
+        a = oracle_mod.pca(X, cfg.K, 1e-9, max_iter, oracle_mod.ALGO_GS, gs_passes=1)
+        b = oracle_mod.pca(X, cfg.K, 1e-9, max_iter, oracle_mod.ALGO_GS, gs_passes=2)
+        assert np.array_equal(a.iters, b.iters)
+        np.testing.assert_allclose(b.lam, a.lam, rtol=1e-12)
+        np.testing.assert_allclose(b.P, a.P, rtol=0, atol=1e-11)
+        I = np.eye(cfg.K)
+        assert np.max(np.abs(b.P.T @ b.P - I)) <= max(np.max(np.abs(a.P.T @ a.P - I)), 1e-15) * 1.5
+        Vn = b.T / b.lam[None, :]
+        assert np.max(np.abs(Vn.T @ Vn - I)) <= 1e-12
+    n1 = oracle_mod.pca(X, 4, 1e-9, 100, oracle_mod.ALGO_NIPALS, gs_passes=1)      # ignored by NIPALS-PCA
+    n2 = oracle_mod.pca(X, 4, 1e-9, 100, oracle_mod.ALGO_NIPALS, gs_passes=2)
+    assert np.array_equal(n1.T, n2.T) and np.array_equal(n1.P, n2.P)
+    with pytest.raises(ValueError):
+        oracle_mod.pca(X, 2, 1e-9, 10, oracle_mod.ALGO_GS, gs_passes=3)

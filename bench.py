@@ -131,7 +131,7 @@ class ClockSampler:
 class GpuProblem:
     """Device buffers + context of one workload (torch: memory and streams only)."""
 
-    def __init__(self, cfg, algo, X_np, K=None, eps=None, max_iter=None):
+    def __init__(self, cfg, algo, X_np, K=None, eps=None, max_iter=None, options=None):
         import torch
         from paper_0811_1081_b200 import binding
         self.torch, self.binding, self.cfg, self.algo = torch, binding, cfg, algo
@@ -140,6 +140,8 @@ class GpuProblem:
         self.eps = cfg.eps if eps is None else eps
         self.max_iter = max_iter or cfg.max_iter
         self.ctx = binding.PcaContext(self.M, self.N, self.K, self.eps, self.max_iter, algo)
+        for opt, val in (options or {}).items():                # plan overrides (--path, --ring-rows, --ring-slots)
+            self.ctx.pca_set_option(opt, val)
         self.X_raw = binding.from_colmajor(X_np)
         self.X = torch.empty_like(self.X_raw)
         self.T = torch.empty((self.K, self.M), dtype=torch.float32, device="cuda")
@@ -349,7 +351,15 @@ def run_cuda_arm(args):
     K = args.components or cfg.K
     eps, max_iter = (0.0, args.fixed_iters) if args.fixed_iters else (cfg.eps, cfg.max_iter)
     pr = inputs.generate(cfg)                                   # replicas only: every rank solves the same seeded problem
-    prob = GpuProblem(cfg, algo, pr.X, K=K, eps=eps, max_iter=max_iter)
+    from paper_0811_1081_b200 import binding as _b
+    plan_opts = {}
+    if args.path:
+        plan_opts[_b.PCA_OPT_PATH] = args.path
+    if args.ring_rows:
+        plan_opts[_b.PCA_OPT_RING_ROWS] = args.ring_rows
+    if args.ring_slots:
+        plan_opts[_b.PCA_OPT_RING_SLOTS] = args.ring_slots
+    prob = GpuProblem(cfg, algo, pr.X, K=K, eps=eps, max_iter=max_iter, options=plan_opts)
     peaks = load_peaks()
 
     def barrier():
@@ -551,6 +561,9 @@ def main():
     ap.add_argument("--no-also", action="store_true")
     ap.add_argument("--also", default="all", help="other configs measured beside the workload: all | comma list of cfg1,cfg2,cfg3,cfg5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", type=int, default=0, help="PCA_OPT_PATH of the main workload (0 = the library's plan)")
+    ap.add_argument("--ring-rows", type=int, default=0, help="path 7: PCA_OPT_RING_ROWS")
+    ap.add_argument("--ring-slots", type=int, default=0, help="path 7: PCA_OPT_RING_SLOTS")
     ap.add_argument("--fig1", action="store_true", help="Fig.-1-shaped sweep (paper's workload) instead of the contract line")
     ap.add_argument("--fig1-sizes", default="512,1024,2048,4096,8192,15000")
     args = ap.parse_args()

@@ -60,7 +60,9 @@ enum {
   PCA_OPT_PATH = 1,     /* 0 = auto; two-sweep kernel: 1 = HBM-streaming, 2 = SMEM-resident;
                            single-sweep kernel (R read once per inner pass): 3 = streaming, 4 = SMEM-resident,
                            5 = register-resident (4*M*N up to ~19 MB on 148 SMs), 6 = one CTA (the matrix in the registers
-                           of one SM: N <= 512, M <= (512/GT)*7 rows with GT = pow2 >= N/8) */
+                           of one SM: N <= 512, M <= (512/GT)*7 rows with GT = pow2 >= N/8),
+                           7 = streaming through a shared-memory ring filled by bulk-async copies (TMA; cp.async.bulk +
+                           mbarrier), Gram-Schmidt coefficients of the scores accumulated during the sweep by helper warps */
   PCA_OPT_CTAS = 2,     /* number of CTAs of the persistent kernel (0 = auto) */
   PCA_OPT_CENTER_MODE = 3, /* 0 = column means (default), 1 = literal eq. (1) mean column */
   PCA_OPT_OWNERS = 5,   /* register-resident kernel: number of slice-owner CTAs (0 = auto; rounded down to a power of two) */
@@ -76,10 +78,12 @@ enum {
   PCA_OPT_OUTPUT = 9,   /* 0 (default): PCA output, T = V Lambda, ||T[:,k]|| = lambda[k];
                            1: SVD output "V, U, Lambda" (eq. 5 :56): T holds the UNIT score vectors V
                            (the epilogue S10 is skipped; NIPALS-PCA: t / lambda), P = U, lambda = Lambda */
-  PCA_OPT_GS_PASSES = 10 /* GS-PCA: classical Gram-Schmidt projections per side per inner pass.  1 (default) = the listings
+  PCA_OPT_GS_PASSES = 10, /* GS-PCA: classical Gram-Schmidt projections per side per inner pass.  1 (default) = the listings
                            (PAPER.md:1025-1026, :1030-1031); 2 = CGS2, "applying it iteratively".  2 is built
                            into the two-sweep kernel only: the plan falls back to paths 1/2, forcing paths 3-6 gives
                            PCA_EUNSUPPORTED.  Ignored for NIPALS-PCA */
+  PCA_OPT_RING_ROWS = 11, /* path 7: rows of R per ring slot (one bulk copy): 0 = auto, 1, 2 or 4 */
+  PCA_OPT_RING_SLOTS = 12 /* path 7: upper bound on the ring slots per row group (0 = auto: what fits, at most 8) */
 };
 
 /* Phase ids of the trace records (pca_trace).  One inner pass of the single-sweep kernel is
@@ -113,6 +117,8 @@ enum {
   PCA_INFO_NUM_SMS = 7,
   PCA_INFO_ROW_GROUP_THREADS = 8, /* single-sweep kernel: threads that share one row of R (0 otherwise) */
   PCA_INFO_OWNERS = 10,     /* slice-owner CTAs (CTAs that combine the partial loads of a column slice) */
+  PCA_INFO_RING_ROWS = 11,  /* path 7: rows per ring slot (0 on other paths) */
+  PCA_INFO_RING_SLOTS = 12, /* path 7: ring slots per row group */
   PCA_INFO_RUN_STATUS = 9   /* SYNCHRONISES the device and reads the status word of the last pca_run: 0 = ok,
                                1 = a cross-CTA exchange wait gave up (results invalid; never in a correct run) */
 };

@@ -19,11 +19,12 @@ PCA_ALGO_GS = 1
 PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED, PCA_EPROTOCOL = range(7)
 
 PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT, PCA_OPT_TEST_MODE = 1, 2, 3, 4, 5, 6, 7
-PCA_OPT_STAGNATION, PCA_OPT_OUTPUT, PCA_OPT_GS_PASSES = 8, 9, 10
+PCA_OPT_STAGNATION, PCA_OPT_OUTPUT, PCA_OPT_GS_PASSES, PCA_OPT_RING_ROWS, PCA_OPT_RING_SLOTS = 8, 9, 10, 11, 12
 (PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT,
- PCA_PATH_REGISTER, PCA_PATH_ONE_CTA) = 0, 1, 2, 3, 4, 5, 6
+ PCA_PATH_REGISTER, PCA_PATH_ONE_CTA, PCA_PATH_TMA_STREAMING) = 0, 1, 2, 3, 4, 5, 6, 7
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
- PCA_INFO_LAUNCHES_PER_RUN, PCA_INFO_NUM_SMS, PCA_INFO_ROW_GROUP_THREADS, PCA_INFO_RUN_STATUS, PCA_INFO_OWNERS) = range(1, 11)
+ PCA_INFO_LAUNCHES_PER_RUN, PCA_INFO_NUM_SMS, PCA_INFO_ROW_GROUP_THREADS, PCA_INFO_RUN_STATUS, PCA_INFO_OWNERS,
+ PCA_INFO_RING_ROWS, PCA_INFO_RING_SLOTS) = range(1, 13)
 
 EXPORTED_SYMBOLS = (
     "pca_create", "pca_set_option", "pca_get_info", "pca_workspace_bytes", "pca_set_workspace",
@@ -119,7 +120,8 @@ class PcaContext:
         return {
             "path": {1: "two-sweep streaming", 2: "two-sweep resident", 3: "single-sweep streaming",
                      4: "single-sweep resident",
-                     5: "single-sweep register-resident", 6: "single-sweep one-CTA"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
+                     5: "single-sweep register-resident", 6: "single-sweep one-CTA",
+                     7: "single-sweep streaming (TMA ring)"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
             "ctas": self.pca_get_info(PCA_INFO_CTAS),
             "threads": self.pca_get_info(PCA_INFO_THREADS),
             "smem_bytes": self.pca_get_info(PCA_INFO_SMEM_BYTES),
@@ -128,6 +130,8 @@ class PcaContext:
             "num_sms": self.pca_get_info(PCA_INFO_NUM_SMS),
             "row_group_threads": self.pca_get_info(PCA_INFO_ROW_GROUP_THREADS),
             "owners": self.pca_get_info(PCA_INFO_OWNERS),
+            "ring_rows": self.pca_get_info(PCA_INFO_RING_ROWS),
+            "ring_slots": self.pca_get_info(PCA_INFO_RING_SLOTS),
         }
 
     def pca_workspace_bytes(self) -> int:

@@ -17,6 +17,7 @@
 #include "pca_one.cuh"
 #include "pca_reg.cuh"
 #include "pca_solve.cuh"
+#include "pca_tma.cuh"
 
 using pca::FusedParams;
 using pca::RegParams;
@@ -52,6 +53,14 @@ const FusedVariant kFusedVariants[] = {
 };
 #undef PCA_FVARIANT
 
+// TMA-staged streaming kernel (pca_tma.cuh): NV float4 per thread per row, RB rows per ring slot
+struct TmaVariant { int nv, rb; fused_kernel_t fn; };
+#define PCA_TVARIANT(NV, RB) {NV, RB, pca::pca_tma_kernel<NV, RB>}
+const TmaVariant kTmaVariants[] = {
+    PCA_TVARIANT(1, 2), PCA_TVARIANT(2, 2), PCA_TVARIANT(3, 2), PCA_TVARIANT(4, 2), PCA_TVARIANT(4, 1), PCA_TVARIANT(4, 4),
+};
+#undef PCA_TVARIANT
+
 }  // namespace
 
 namespace pca {
@@ -85,7 +94,7 @@ struct pca_ctx {
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
-  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1;
+  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -99,6 +108,9 @@ struct pca_ctx {
   const Variant* variant = nullptr;
   SolveParams prm{};
   const FusedVariant* fvariant = nullptr;
+  fused_kernel_t ffn = nullptr;      // the kernel of paths 3, 4, 7
+  int ring_rows = 0;
+  size_t ws_off_vrm = 0;
   FusedParams fprm{};
   size_t ws_off_rrm = 0, ws_off_xchg = 0, ws_xchg_bytes = 0, ws_off_qx = 0, ws_off_sbx = 0, ws_off_ax = 0, ws_off_px = 0,
          ws_off_nx = 0, ws_off_pown = 0, ws_off_wown = 0, ws_off_status = 0, ws_off_cnt = 0, ws_off_trace = 0;
@@ -192,6 +204,8 @@ int make_fused_plan(pca_ctx* c, int want) {
   const int NV = (int)ceil_div(N, 4LL * GT);
   const int ldr = 4 * GT * NV;
   const int g_min = (int)ceil_div(N, pca::kThreads);
+  int tma_rb = 0;                                                     // > 0: TMA plan with tma_rb rows per ring slot
+  bool tma_no_cache = false;
   auto carve_fused = [&](int resident, int G, FusedParams* p) -> size_t {
     p->G = G;
     p->Mb = (int)ceil_div(M, G);
@@ -219,6 +233,7 @@ int make_fused_plan(pca_ctx* c, int want) {
     const size_t panel = (size_t)p->Ns * p->Kpad * 4;
     const size_t slab_bytes = resident ? (size_t)p->Mb * (size_t)ldr * 4 : 0;
     p->cache_pw = (off + 2 * panel + slab_bytes <= (size_t)c->smem_optin && 2 * panel <= (size_t)64 * 1024) ? 1 : 0;
+    if (tma_rb && (tma_no_cache || 2 * panel > (size_t)32 * 1024)) p->cache_pw = 0;
     p->off_pc = take(p->cache_pw ? panel : 0);
     p->off_wc = take(p->cache_pw ? panel : 0);
     p->off_slab = take(resident ? (size_t)p->Mb * (size_t)ldr * 4 : 0);
@@ -226,6 +241,26 @@ int make_fused_plan(pca_ctx* c, int want) {
     p->Mbp = (int)round_up(p->Mb, 32);
     p->Ksm = 0;
     p->off_vc = (int)off;
+    p->SG = 0;
+    if (tma_rb) {
+      // ring: NG groups x SG slots of tma_rb rows; everything that is left of the shared memory, at most 8 slots per group
+      p->off_hb = take((size_t)pca::kHelperWarps * p->Kpad * 4);
+      p->off_cmd = take(16);
+      p->off_prog = take((size_t)(pca::kThreads / GT) * 4);
+      const int NG = pca::kThreads / GT;
+      p->off_mbar = take((size_t)NG * 8 * 8);
+      off = (size_t)round_up((long long)off, 128);
+      const size_t slot = (size_t)tma_rb * ldr * 4;
+      long long sg = ((long long)c->smem_optin - (long long)off) / (long long)(slot * NG);
+      const long long need = ceil_div(ceil_div(p->Mb, tma_rb), NG);        // batches per group and sweep
+      if (sg > 8) sg = 8;
+      if (sg > need + 1) sg = need + 1;
+      if (c->opt_ring_slots > 0 && sg > c->opt_ring_slots) sg = c->opt_ring_slots;
+      if (sg < 1) return (size_t)c->smem_optin + 1;                         // does not fit
+      p->SG = (int)sg;
+      p->off_ring = take((size_t)NG * sg * slot);
+      return off;
+    }
     // (streaming plan: not beyond 100 KB in total -- the sweep keeps 128 KB of loads in flight per SM and those need L1 lines;
     //  measured on config 4: with all 227 KB as shared memory the sweep is 33 % slower)
     const long long cap = resident ? (long long)c->smem_optin : (100LL * 1024 < c->smem_optin ? 100LL * 1024 : (long long)c->smem_optin);
@@ -257,7 +292,27 @@ int make_fused_plan(pca_ctx* c, int want) {
     return var != nullptr;
   };
   bool ok = false;
-  if (want == 0 || want == 4) {
+  const TmaVariant* tvar = nullptr;
+  if (want == 7) {
+    const int G = c->opt_ctas > 0 ? c->opt_ctas : sms;
+    const int prefer[3] = {c->opt_ring_rows > 0 ? c->opt_ring_rows : 2, 1, 4};
+    for (int pi = 0; pi < (c->opt_ring_rows > 0 ? 1 : 3) && !ok; ++pi)
+      for (int nc = 0; nc < 2 && !ok; ++nc) {
+        tma_rb = prefer[pi];
+        tma_no_cache = nc == 1;
+        tvar = nullptr;
+        for (const TmaVariant& v : kTmaVariants)
+          if (v.nv == NV && v.rb == tma_rb) tvar = &v;
+        if (!tvar) continue;
+        int Gc = G < g_min ? g_min : G;
+        if (Gc > sms || g_min > sms) continue;
+        smem = carve_fused(0, Gc, &p);
+        if (smem <= (size_t)c->smem_optin && (p.SG >= 2 || (pi == 2 && nc == 1) || c->opt_ring_rows > 0)) ok = true;
+      }
+    if (!ok) return PCA_EUNSUPPORTED;
+    path = 7;
+  }
+  if (!ok && (want == 0 || want == 4)) {
     int G = c->opt_ctas > 0 ? c->opt_ctas : ((size_t)M * (size_t)ldr * 4 <= (size_t)160 * 1024 ? 1 : sms);
     ok = try_plan(1, G);
     if (!ok && c->opt_ctas == 0 && G != sms) ok = try_plan(1, sms);
@@ -269,10 +324,12 @@ int make_fused_plan(pca_ctx* c, int want) {
     if (!ok) return PCA_EUNSUPPORTED;
     path = 3;
   }
-  cudaError_t e = cudaFuncSetAttribute(var->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  fused_kernel_t fn = path == 7 ? tvar->fn : var->fn;
+  const int nthreads = path == 7 ? pca::kTmaThreads : pca::kThreads;
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return cuda_fail(c, e);
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, var->fn, pca::kThreads, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, nthreads, smem);
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
 
@@ -294,10 +351,13 @@ int make_fused_plan(pca_ctx* c, int want) {
   c->ws_off_cnt = take(1024);
   c->ws_xchg_bytes = off - c->ws_off_xchg;
   c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1) * 8 : 0);
+  c->ws_off_vrm = take(path == 7 && c->algo == PCA_ALGO_GS ? (size_t)M * p.Kpad * 4 : 0);
   p.trace_cap = c->opt_trace;
   c->ws_bytes = off;
   c->fprm = p;
   c->fvariant = var;
+  c->ffn = fn;
+  c->ring_rows = tma_rb;
   c->smem_bytes = smem;
   c->path = path;
   c->planned = true;
@@ -480,7 +540,7 @@ int make_plan(pca_ctx* c) {
     if (rc == PCA_OK || c->opt_path != 0) return rc;
     if (rc == PCA_ECUDA) return rc;
   }
-  if (!cgs2 && (c->opt_path == 0 || c->opt_path == 3 || c->opt_path == 4)) {
+  if (!cgs2 && (c->opt_path == 0 || c->opt_path == 3 || c->opt_path == 4 || c->opt_path == 7)) {
     const int rc = make_fused_plan(c, c->opt_path);
     if (rc == PCA_OK || c->opt_path != 0) return rc;
     if (rc == PCA_ECUDA) return rc;
@@ -559,7 +619,7 @@ int make_plan(pca_ctx* c) {
 int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
   switch (option) {
     case PCA_OPT_PATH:
-      if (value < 0 || value > 6) return PCA_EINVAL;
+      if (value < 0 || value > 7) return PCA_EINVAL;
       c->opt_path = (int)value;
       break;
     case PCA_OPT_CTAS:
@@ -597,6 +657,14 @@ int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
     case PCA_OPT_GS_PASSES:
       if (value < 1 || value > 2) return PCA_EINVAL;
       c->opt_gs_passes = (int)value;
+      break;
+    case PCA_OPT_RING_ROWS:
+      if (value != 0 && value != 1 && value != 2 && value != 4) return PCA_EINVAL;
+      c->opt_ring_rows = (int)value;
+      break;
+    case PCA_OPT_RING_SLOTS:
+      if (value < 0 || value > 8) return PCA_EINVAL;
+      c->opt_ring_slots = (int)value;
       break;
     default:
       return PCA_EINVAL;
@@ -652,11 +720,13 @@ int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
     case PCA_INFO_PATH: *value = c->path; break;
     case PCA_INFO_CTAS: *value = c->path == 6 ? 1 : c->path == 5 ? c->rprm.G : (c->path >= 3 ? c->fprm.G : c->prm.G); break;
     case PCA_INFO_OWNERS: *value = c->path == 6 ? 1 : c->path == 5 ? c->rprm.Gs : (c->path >= 3 ? c->fprm.Gs : c->prm.Gs); break;
-    case PCA_INFO_THREADS: *value = pca::kThreads; break;
+    case PCA_INFO_THREADS: *value = c->path == 7 ? pca::kTmaThreads : pca::kThreads; break;
     case PCA_INFO_SMEM_BYTES: *value = (int64_t)c->smem_bytes; break;
     case PCA_INFO_ROWS_PER_CTA: *value = c->path == 6 ? c->oprm.M : c->path == 5 ? c->rprm.Mb : (c->path >= 3 ? c->fprm.Mb : c->prm.Mb); break;
     case PCA_INFO_LAUNCHES_PER_RUN: *value = c->path >= 3 ? 3 : 1; break;
-    case PCA_INFO_ROW_GROUP_THREADS: *value = c->path >= 5 ? c->r_gt : (c->path >= 3 ? c->fprm.GT : 0); break;
+    case PCA_INFO_ROW_GROUP_THREADS: *value = (c->path == 5 || c->path == 6) ? c->r_gt : (c->path >= 3 ? c->fprm.GT : 0); break;
+    case PCA_INFO_RING_ROWS: *value = c->path == 7 ? c->ring_rows : 0; break;
+    case PCA_INFO_RING_SLOTS: *value = c->path == 7 ? c->fprm.SG : 0; break;
     case PCA_INFO_NUM_SMS: *value = c->num_sms; break;
     case PCA_INFO_RUN_STATUS: {
       *value = 0;
@@ -763,14 +833,15 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     p.status = reinterpret_cast<unsigned*>(ws + c->ws_off_status);
     p.cnt = reinterpret_cast<unsigned*>(ws + c->ws_off_cnt);
     p.trace = reinterpret_cast<unsigned long long*>(ws + c->ws_off_trace);
+    p.Vrm = reinterpret_cast<float*>(ws + c->ws_off_vrm);
     PCA_CUDA(c, cudaMemsetAsync(ws + c->ws_off_xchg, 0, c->ws_xchg_bytes, st));   // sequence numbers start at 0
     if (p.trace_cap > 0) PCA_CUDA(c, cudaMemsetAsync(p.trace, 0, 8, st));
     const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
     pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X
     PCA_CUDA(c, cudaGetLastError());
     void* fargs[] = {&p};
-    PCA_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(c->fvariant->fn), dim3((unsigned)p.G),
-                                            dim3(pca::kThreads), fargs, c->smem_bytes, st));
+    PCA_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(c->ffn), dim3((unsigned)p.G),
+                                            dim3(c->path == 7 ? pca::kTmaThreads : pca::kThreads), fargs, c->smem_bytes, st));
     const dim3 ogrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(c->N, 32));
     pca::pca_transpose_out_kernel<<<ogrid, 256, 0, st>>>(p.Rrm, reinterpret_cast<float*>(ws),
                                                          T + (size_t)(c->K - 1) * (size_t)c->M,

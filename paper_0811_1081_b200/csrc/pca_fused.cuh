@@ -75,6 +75,10 @@ struct FusedParams {
   unsigned* cnt;            // arrival-counter hints of the three hops, 64 words apart (relaxed; see hop_arrive/hop_wait)
   unsigned long long* trace;  // optional phase trace (PCA_OPT_TRACE): [0] = records written, then records
   int trace_cap;              // capacity in records (0 = off)
+  // TMA-staged streaming kernel (pca_tma.cuh, path 7)
+  float* Vrm;                 // [M][Kpad] row-major copy of the unit score vectors (helper warps: B-partials during the sweep)
+  int SG;                     // ring slots per row group
+  int off_ring, off_mbar, off_hb, off_cmd, off_prog;
   // shared-memory carve-up (byte offsets)
   int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_pc, off_wc,
       off_slab, off_vc;

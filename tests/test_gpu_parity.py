@@ -123,6 +123,17 @@ SMALL_CASES = [
     (1, 100, 200, 6, 6, 0),         # M < N, 32 threads per row
     (4, 400, 64, 64, 6, 0),         # 7 rows per thread, K = N
     (2, 56, 500, 10, 6, 0),         # 64 threads per row, collinear columns
+    # TMA-staged streaming kernel (path 7): bulk-async copies into per-group rings, helper warps for the B-partials
+    (0, 256, 64, 8, 7, 0),          # 148 CTAs, most own 2 rows (one ring slot, partial), some none
+    (0, 256, 64, 8, 7, 3),          # 3 CTAs x 86 rows: 16 row groups of 32 threads, ragged last batch
+    (1, 1000, 200, 6, 7, 0),        # row group = 32 threads, 2 float4 per thread, padded columns
+    (1, 1027, 131, 5, 7, 20),       # M % 4 != 0 and N % 4 != 0; odd rows per CTA (a one-row last batch)
+    (1, 3000, 700, 12, 7, 0),       # row group = 64 threads (cross-warp row reduction), NV = 3
+    (2, 2048, 512, 20, 7, 9),       # collinear columns; 228 rows per CTA: the ring wraps many times per sweep
+    (3, 8192, 256, 16, 7, 0),       # tall
+    (3, 4096, 2048, 10, 7, 0),      # row group = 128 threads (config-4 column count)
+    (2, 1024, 4096, 6, 7, 0),       # row group = 256 threads (config-3 column count), M < N
+    (4, 1024, 64, 64, 7, 4),        # K = N full decomposition, 256 rows per CTA
 ]
 
 
@@ -226,8 +237,8 @@ def test_paths_agree_and_are_deterministic(binding):
     each plan is bitwise reproducible run to run (fixed-order reductions)."""
     cfg = inputs.scaled(inputs.config(1), 1536, 384, K=6)
     pr = inputs.generate(cfg)
-    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2, 3, 3, 4, 4, 5, 5)]
-    for a, b in ((0, 1), (2, 3), (4, 5), (6, 7), (8, 9)):
+    runs = [binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, path=p) for p in (1, 1, 2, 2, 3, 3, 4, 4, 5, 5, 7, 7)]
+    for a, b in ((0, 1), (2, 3), (4, 5), (6, 7), (8, 9), (10, 11)):
         for key in ("T", "P", "lam", "iters"):
             np.testing.assert_array_equal(runs[a][key], runs[b][key])
     for r in runs[1:]:
@@ -272,6 +283,8 @@ FIXED_PASS_CASES = [
     (2, 2048, 512, 20, 5, 0), (2, 2048, 512, 20, 3, 0), (2, 2048, 512, 20, 1, 0),
     (4, 1024, 64, 64, 5, 0), (4, 1024, 64, 64, 4, 0), (4, 400, 64, 64, 6, 0), (4, 1024, 64, 64, 3, 0),
     (3, 4096, 2048, 10, 3, 0), (2, 1024, 4096, 6, 3, 0), (1, 3000, 700, 12, 5, 0),
+    (0, 256, 64, 8, 7, 3), (1, 1027, 131, 5, 7, 20), (2, 2048, 512, 20, 7, 9), (4, 1024, 64, 64, 7, 4), (3, 4096, 2048, 10, 7, 0),
+    (2, 1024, 4096, 6, 7, 0),
 ]
 
 
@@ -365,7 +378,7 @@ def test_eps_zero_runs_exactly_max_iter(binding):
     cfg = inputs.scaled(inputs.config(0), 256, 64, K=3)
     pr = inputs.generate(cfg)
     for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
-        for path in (0, 1, 2, 3, 4, 5, 6):
+        for path in (0, 1, 2, 3, 4, 5, 6, 7):
             got = binding.fit(pr.X, 3, 0.0, 7, algo, path=path)
             assert got["iters"].tolist() == [7, 7, 7]
         got = binding.fit(pr.X, 3, 0.0, 1, algo)               # a single pass per component
@@ -407,7 +420,7 @@ def test_golden_gs_3x3_one_pass_on_gpu(binding):
     scores-side coefficient B (S6), deflation (S9), epilogue (S10) -- on every plan, at fp32 tolerance."""
     g = json.load(open(os.path.join(GOLD, "worked_gs_3x3.json")))
     X = np.asfortranarray(np.array(g["X_rows"], dtype=np.float32))
-    for path in (0, 1, 2, 3, 4, 5, 6):
+    for path in (0, 1, 2, 3, 4, 5, 6, 7):
         got = binding.fit(X, g["K"], g["eps"], g["max_iter"], inputs.ALGO_GS, center=False, path=path, want_residual=True)
         assert got["iters"].tolist() == g["iters"], path
         for k in range(2):
@@ -427,7 +440,7 @@ def test_stagnation_option(binding):
     cfg = inputs.scaled(inputs.config(0), 256, 64, K=2)
     pr = inputs.generate(cfg)
     eps, J = 1e-3, 14
-    for path in (0, 1, 2, 3, 4, 5, 6):
+    for path in (0, 1, 2, 3, 4, 5, 6, 7):
         for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
             lam_seq = [float(binding.fit(pr.X, 1, 0.0, j, algo, path=path, options={binding.PCA_OPT_STAGNATION: 0})["lam"][0])
                        for j in range(1, J + 1)]
@@ -535,7 +548,7 @@ def test_absolute_test_mode(binding, oracle_mod):
     a = g["absolute_test"]
     X = np.asfortranarray(np.array(g["X_rows"], dtype=np.float32))
     nrm = np.sqrt(a["norm_sq"])
-    for path in (0, 1, 2, 3, 4, 5, 6):
+    for path in (0, 1, 2, 3, 4, 5, 6, 7):
         got = binding.fit(X, 1, a["eps"], g["max_iter"], inputs.ALGO_NIPALS, center=False, path=path, test_mode=1)
         assert got["iters"].tolist() == a["iters"], path
         np.testing.assert_allclose(got["lam"][0], np.sqrt(a["lambda_sq_num"] / a["lambda_sq_den"]), rtol=1e-6)

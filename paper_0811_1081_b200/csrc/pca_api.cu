@@ -94,7 +94,7 @@ struct pca_ctx {
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
-  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0;
+  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0, opt_l2_tail = -1;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -357,6 +357,7 @@ int make_fused_plan(pca_ctx* c, int want) {
   c->fprm = p;
   c->fvariant = var;
   c->ffn = fn;
+  c->fprm.l2_tail = c->opt_l2_tail >= 0 ? c->opt_l2_tail : 100;       // measured: 0 .. 260 permille within 1-2 % of each other
   c->ring_rows = tma_rb;
   c->smem_bytes = smem;
   c->path = path;
@@ -665,6 +666,10 @@ int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
     case PCA_OPT_RING_SLOTS:
       if (value < 0 || value > 8) return PCA_EINVAL;
       c->opt_ring_slots = (int)value;
+      break;
+    case PCA_OPT_L2_TAIL:
+      if (value < -1 || value > 1000) return PCA_EINVAL;
+      c->opt_l2_tail = (int)value;
       break;
     default:
       return PCA_EINVAL;

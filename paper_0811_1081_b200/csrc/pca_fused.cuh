@@ -78,6 +78,7 @@ struct FusedParams {
   // TMA-staged streaming kernel (pca_tma.cuh, path 7)
   float* Vrm;                 // [M][Kpad] row-major copy of the unit score vectors (helper warps: B-partials during the sweep)
   int SG;                     // ring slots per row group
+  int l2_tail;                // permille of a sweep's batches fetched with L2 evict_last (PCA_OPT_L2_TAIL)
   int off_ring, off_mbar, off_hb, off_cmd, off_prog;
   // shared-memory carve-up (byte offsets)
   int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_pc, off_wc,

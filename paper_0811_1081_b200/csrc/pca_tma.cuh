@@ -66,6 +66,21 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
+// ... with an L2 eviction-priority hint (createpolicy)
+__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, unsigned bytes, void* bar, unsigned long long pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+  unsigned long long p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+  unsigned long long p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void st_release_cta(unsigned* p, unsigned v) {
   asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
@@ -115,25 +130,39 @@ struct Ring {
   const float* Rb;          // the CTA's rows of the row-major residual
   int SG, ldr, mb, nb, g, NG;
   unsigned* status;
-  unsigned cons;            // batches consumed (all threads of the group)
-  unsigned iss;             // batches issued (leader)
-  int iss_sw, iss_bq;       // stream position of the next batch to issue (leader)
+  // running indices instead of count % SG, count / SG (integer division is a long serial sequence on the leader's path)
+  int cons_slot;            // slot of the next batch to consume (all threads of the group)
+  unsigned cons_par;        // its mbarrier phase parity
+  unsigned cons;            // batches consumed
+  int iss_slot;             // leader: slot of the next batch to issue
+  int inflight;             // leader: issued and not yet consumed
+  int iss_sw, iss_bq;       // leader: stream position of the next batch to issue
+  // L2 residency control: the last `tail_from..nb` batch positions of a sweep are the head of the next one (opposite row
+  // order); they are fetched with evict_last, everything else with evict_first, so that the 126 MB L2 keeps exactly the
+  // rows that are read again soonest instead of an LRU mix of the stream.  tail_from >= nb: no hints.
+  int tail_from;
+  unsigned long long pol_keep, pol_stream;
 
-  __device__ __forceinline__ float* slot_ptr(unsigned n) const { return slots + (size_t)(n % (unsigned)SG) * RB * ldr; }
-  __device__ __forceinline__ void wait_next() const {                      // batch `cons` has landed
-    mbar_wait(full + (cons % (unsigned)SG), (cons / (unsigned)SG) & 1u, status);
+  __device__ __forceinline__ const float* cur_slot() const { return slots + (size_t)cons_slot * (RB * ldr); }
+  __device__ __forceinline__ void wait_next() const { mbar_wait(full + cons_slot, cons_par, status); }   // batch has landed
+  __device__ __forceinline__ void consumed() {                             // all threads of the group, after the batch is in registers
+    ++cons;
+    if (++cons_slot == SG) { cons_slot = 0; cons_par ^= 1u; }
   }
   // leader: issue copies while a slot is free and the stream position is within sweeps <= limit_sw
   __device__ __forceinline__ void top_up(int limit_sw) {
-    while (iss - cons < (unsigned)SG && iss_sw <= limit_sw && g < nb) {
+    while (inflight < SG && iss_sw <= limit_sw && g < nb) {
       const int bi = (iss_sw & 1) ? (nb - 1 - iss_bq) : iss_bq;
       const int r0 = bi * RB;
       const int rows = min(RB, mb - r0);
       const unsigned bytes = (unsigned)rows * (unsigned)ldr * 4u;
-      unsigned long long* bar = full + (iss % (unsigned)SG);
+      unsigned long long* bar = full + iss_slot;
       mbar_expect_tx(bar, bytes);
-      bulk_g2s(slot_ptr(iss), Rb + (size_t)r0 * ldr, bytes, bar);
-      ++iss;
+      if (tail_from >= nb) bulk_g2s(slots + (size_t)iss_slot * (RB * ldr), Rb + (size_t)r0 * ldr, bytes, bar);
+      else bulk_g2s_hint(slots + (size_t)iss_slot * (RB * ldr), Rb + (size_t)r0 * ldr, bytes, bar,
+                         iss_bq >= tail_from ? pol_keep : pol_stream);
+      ++inflight;
+      if (++iss_slot == SG) iss_slot = 0;
       iss_bq += NG;
       if (iss_bq >= nb) { iss_bq = g; ++iss_sw; }
     }
@@ -199,24 +228,30 @@ __device__ __forceinline__ void group_row_sums(float (&part)[RB], float (&tt)[RB
 // the second product.  Leaves qs[g][ldr], ttil_s[rows], sgrp[g] = sum t~^2 (fp64); ends with cta_sync().
 template <int NV, int RB>
 __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB>& rg, int sw, const float* p_s,
-                                                 float* ttil_s, float* qs, float* red_s, double* sgrp, unsigned* prog_s) {
+                                                 float* ttil_s, float* qs, float* red_s, double* sgrp, unsigned* prog_s,
+                                                 long long* prof = nullptr) {
   const int GT = prm.GT, NG = kThreads / GT, WG = GT >> 5, ldr = prm.ldr;
+#ifdef PCA_TMA_PROFILE
+  long long pc0 = 0, pc1 = 0, pc2 = 0, pc3 = 0, tq = clock64();
+#define PROF_STEP(acc) { const long long tnow = clock64(); acc += tnow - tq; tq = tnow; }
+#else
+#define PROF_STEP(acc)
+#endif
   const int tid = threadIdx.x, g = tid / GT, gl = tid - g * GT, lane = tid & 31, wg = gl >> 5;
-  float4 pr[NV], q[NV];
-#pragma unroll
-  for (int v = 0; v < NV; ++v) {
-    pr[v] = *reinterpret_cast<const float4*>(p_s + 4 * (gl + GT * v));
-    q[v] = make_float4(0.f, 0.f, 0.f, 0.f);
-  }
+  float4 q[NV];                                                            // (p is re-read from shared memory per batch:
+#pragma unroll                                                             //  16 registers less, no spills in the loop)
+  for (int v = 0; v < NV; ++v) q[v] = make_float4(0.f, 0.f, 0.f, 0.f);
   double sacc = 0.0;
   int parity = 0;
   const bool rev = (sw & 1) != 0;
+  const int gl2 = GT >= 64 ? 32 : 0;                                      // thread of the group that records t~ and |t~|^2
   for (int bq = g; bq < rg.nb; bq += NG) {
     const int bi = rev ? (rg.nb - 1 - bq) : bq;
     const int r0 = bi * RB;
     const int rows = min(RB, rg.mb - r0);
     rg.wait_next();
-    const float* sl = rg.slot_ptr(rg.cons);
+    PROF_STEP(pc0)
+    const float* sl = rg.cur_slot();
     float4 x[RB][NV];
 #pragma unroll
     for (int i = 0; i < RB; ++i) {
@@ -228,16 +263,22 @@ __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB
     }
     float part[RB], tt[RB];
 #pragma unroll
-    for (int i = 0; i < RB; ++i) {
-      float a = 0.f;
+    for (int i = 0; i < RB; ++i) part[i] = 0.f;
 #pragma unroll
-      for (int v = 0; v < NV; ++v) a = dot4(x[i][v], pr[v], a);
-      part[i] = a;
+    for (int v = 0; v < NV; ++v) {
+      const float4 pv = *reinterpret_cast<const float4*>(p_s + 4 * (gl + GT * v));
+#pragma unroll
+      for (int i = 0; i < RB; ++i) part[i] = dot4(x[i][v], pv, part[i]);
     }
     group_row_sums<RB>(part, tt, WG, g, GT, wg, lane, red_s, parity);     // every thread of the group has read the slot
-    ++rg.cons;
+    rg.consumed();
+    PROF_STEP(pc1)
     if (gl == 0) {
+      --rg.inflight;
       rg.top_up(sw + 1);                                                  // refill: this sweep, then the head of the next
+    }
+    PROF_STEP(pc2)
+    if (gl == gl2) {                                                      // (not the refilling thread when the group has 2+ warps)
 #pragma unroll
       for (int i = 0; i < RB; ++i)
         if (i < rows) {
@@ -250,10 +291,14 @@ __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB
     for (int i = 0; i < RB; ++i)
 #pragma unroll
       for (int v = 0; v < NV; ++v) axpy4(q[v], x[i][v], tt[i]);
+    PROF_STEP(pc3)
   }
+#ifdef PCA_TMA_PROFILE
+  if (prof) { prof[0] = pc0; prof[1] = pc1; prof[2] = pc2; prof[3] = pc3; }
+#endif
 #pragma unroll
   for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q[v];
-  if (gl == 0) sgrp[g] = sacc;
+  if (gl == gl2) sgrp[g] = sacc;
   cta_sync();
 }
 
@@ -277,7 +322,7 @@ __device__ __forceinline__ void sweep_loads_ring(const FusedParams& prm, Ring<RB
     const int r0 = bi * RB;
     const int rows = min(RB, rg.mb - r0);
     rg.wait_next();
-    const float* sl = rg.slot_ptr(rg.cons);
+    const float* sl = rg.cur_slot();
     float4 x[RB][NV];
 #pragma unroll
     for (int i = 0; i < RB; ++i) {
@@ -305,8 +350,11 @@ __device__ __forceinline__ void sweep_loads_ring(const FusedParams& prm, Ring<RB
     }
     if (GT == 32) __syncwarp();                                           // every thread of the group has read the slot
     else named_bar_sync(1 + g, GT);                                       // (its values went through the FMAs above)
-    ++rg.cons;
-    if (gl == 0) rg.top_up(DEFL ? sw : sw + 1);                           // a writing sweep is not overtaken (file header)
+    rg.consumed();
+    if (gl == 0) {
+      --rg.inflight;
+      rg.top_up(DEFL ? sw : sw + 1);                                      // a writing sweep is not overtaken (file header)
+    }
   }
 #pragma unroll
   for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q[v];
@@ -362,7 +410,8 @@ __device__ __forceinline__ void helper_main(const FusedParams& prm, int mb, long
             const unsigned need = (unsigned)sw * (unsigned)((nb - gq + NG - 1) / NG) + (unsigned)(bq / NG) + 1u;
             unsigned spins = 0;
             while ((int)(ld_acquire_cta(prog_s + gq) - need) < 0) {         // the row group has not finished this batch yet
-              if (++spins > (kSpinLimit << 4)) { *prm.status = 1u; break; }
+              __nanosleep(64);                                             // (do not compete with the row groups for issue slots)
+              if (++spins > (kSpinLimit << 2)) { *prm.status = 1u; break; }
             }
             const int r0 = (rev ? (nb - 1 - bq) : bq) * RB;
 #pragma unroll
@@ -426,10 +475,14 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   fence_proxy_async();
   __syncthreads();                                         // all kTmaThreads threads, once
+  // register file: 20 warps = 5 per SM sub-partition = 96 registers per thread at launch; the helper warp group hands
+  // registers over to the four compute warp groups (the launch holds 5 x 96 = 480 per lane slot: 4 x 104 + 64 = 480; asking for more would wait forever)
   if (w >= kWarps) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
     helper_main<RB>(prm, mb, m0, ttil_s, hb_s, cmd_s, prog_s);
     return;
   }
+  asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
 
   const int npx = Gs * Ns;                                 // exchanged length of p (>= N)
   const int SBw = 2 + Kpad;
@@ -457,7 +510,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
     rg.slots = ring_s + (size_t)g * SG * RB * ldr;
     rg.full = mbar_s + g * SG;
     rg.Rb = Rb; rg.SG = SG; rg.ldr = ldr; rg.mb = mb; rg.nb = (mb + RB - 1) / RB; rg.g = g; rg.NG = NG;
-    rg.cons = 0; rg.iss = 0; rg.iss_sw = 0; rg.iss_bq = g; rg.status = status;
+    rg.cons = 0; rg.cons_slot = 0; rg.cons_par = 0u; rg.iss_slot = 0; rg.inflight = 0; rg.iss_sw = 0; rg.iss_bq = g; rg.status = status;
+    rg.tail_from = prm.l2_tail > 0 ? rg.nb - (int)(((long long)rg.nb * prm.l2_tail) / 1000) : rg.nb;
+    rg.pol_keep = l2_policy_evict_last();
+    rg.pol_stream = l2_policy_evict_first();
     if (tid - g * GT == 0) rg.top_up(0);                   // the head of the first sweep is on its way
   }
   int sw = 0;                                              // sweeps done (loads sweeps included): row order of the next one
@@ -674,7 +730,14 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
       {
         const unsigned npar = seq & 1u;
         if (gsk) bar_arrive(BAR_HSTART, kTmaThreads);                         // the helpers start following the row groups
+#ifdef PCA_TMA_PROFILE
+        long long prof[4] = {0, 0, 0, 0};
+        sweep_fused_ring<NV, RB>(prm, rg, sw, p_s, ttil_s, qs, red_s, sgrp, prog_s, prof);
+        if (prm.trace_cap > 0 && b == 0 && tid == 0)
+          for (int q4 = 0; q4 < 4 && tn < prm.trace_cap; ++q4) { prm.trace[1 + tn] = ((unsigned long long)(20 + q4) << 56) | (unsigned long long)prof[q4]; ++tn; }
+#else
         sweep_fused_ring<NV, RB>(prm, rg, sw, p_s, ttil_s, qs, red_s, sgrp, prog_s);
+#endif
         ++sw;
         trace_mark(prm, tn, TR_SWEEP);
         publish_q_ll(prm, qs, prm.Qx + (size_t)npar * Gs * G * Ns, b, seq);
@@ -748,9 +811,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
   if (tid == 0) cmd_s[0] = HCMD_EXIT;
   bar_arrive(BAR_HSTART, kTmaThreads);
   if (tid == rg.g * GT) {                                  // (only the group leaders know how many copies they issued)
-    while (rg.cons < rg.iss) {
+    while (rg.inflight > 0) {
       rg.wait_next();
-      ++rg.cons;
+      rg.consumed();
+      --rg.inflight;
     }
   }
   // ---- S10: GS-PCA  T <- V Lambda; skipped for the SVD output V, U, Lambda ----

@@ -359,8 +359,6 @@ def run_cuda_arm(args):
         plan_opts[_b.PCA_OPT_RING_ROWS] = args.ring_rows
     if args.ring_slots:
         plan_opts[_b.PCA_OPT_RING_SLOTS] = args.ring_slots
-    if args.l2_tail >= 0:
-        plan_opts[_b.PCA_OPT_L2_TAIL] = args.l2_tail
     prob = GpuProblem(cfg, algo, pr.X, K=K, eps=eps, max_iter=max_iter, options=plan_opts)
     peaks = load_peaks()
 
@@ -566,7 +564,6 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="PCA_OPT_PATH of the main workload (0 = the library's plan)")
     ap.add_argument("--ring-rows", type=int, default=0, help="path 7: PCA_OPT_RING_ROWS")
     ap.add_argument("--ring-slots", type=int, default=0, help="path 7: PCA_OPT_RING_SLOTS")
-    ap.add_argument("--l2-tail", type=int, default=-1, help="path 7: PCA_OPT_L2_TAIL (permille)")
     ap.add_argument("--fig1", action="store_true", help="Fig.-1-shaped sweep (paper's workload) instead of the contract line")
     ap.add_argument("--fig1-sizes", default="512,1024,2048,4096,8192,15000")
     args = ap.parse_args()

@@ -83,10 +83,7 @@ enum {
                            into the two-sweep kernel only: the plan falls back to paths 1/2, forcing paths 3-6 gives
                            PCA_EUNSUPPORTED.  Ignored for NIPALS-PCA */
   PCA_OPT_RING_ROWS = 11, /* path 7: rows of R per ring slot (one bulk copy): 0 = auto, 1, 2 or 4 */
-  PCA_OPT_RING_SLOTS = 12, /* path 7: upper bound on the ring slots per row group (0 = auto: what fits, at most 8) */
-  PCA_OPT_L2_TAIL = 13    /* path 7: permille (0..1000) of the rows of a sweep, counted from its END, that are fetched with the
-                            L2 eviction priority evict_last (the rest evict_first): alternate sweeps run in opposite row order,
-                            so those rows are the first ones the next sweep reads.  0 = no hints, -1 = default */
+  PCA_OPT_RING_SLOTS = 12 /* path 7: upper bound on the ring slots per row group (0 = auto: what fits, at most 8) */
 };
 
 /* Phase ids of the trace records (pca_trace).  One inner pass of the single-sweep kernel is

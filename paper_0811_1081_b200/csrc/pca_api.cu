@@ -94,7 +94,7 @@ struct pca_ctx {
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
-  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0, opt_l2_tail = -1;
+  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -110,7 +110,7 @@ struct pca_ctx {
   const FusedVariant* fvariant = nullptr;
   fused_kernel_t ffn = nullptr;      // the kernel of paths 3, 4, 7
   int ring_rows = 0;
-  size_t ws_off_vrm = 0;
+  size_t ws_off_vrm = 0, ws_off_pfx = 0, ws_off_nfx = 0;
   FusedParams fprm{};
   size_t ws_off_rrm = 0, ws_off_xchg = 0, ws_xchg_bytes = 0, ws_off_qx = 0, ws_off_sbx = 0, ws_off_ax = 0, ws_off_px = 0,
          ws_off_nx = 0, ws_off_pown = 0, ws_off_wown = 0, ws_off_status = 0, ws_off_cnt = 0, ws_off_trace = 0;
@@ -224,10 +224,10 @@ int make_fused_plan(pca_ctx* c, int want) {
     p->off_qs = take((size_t)pca::kThreads * 4 * NV * 4);
     p->off_red = take((size_t)2 * pca::kWarps * pca::kRB * 4);
     p->off_sgrp = take((size_t)(pca::kThreads / GT) * 8);
-    p->off_B = take((size_t)(2 + p->Kpad) * 8);
+    p->off_B = take((size_t)(4 + p->Kpad) * 8);
     p->off_A = take((size_t)p->Kpad * 8);
     p->off_scr = take((size_t)pca::kThreads * 8);
-    p->off_praw = take((size_t)p->Ns * 8);
+    p->off_praw = take((size_t)2 * p->Ns * 8);
     p->off_lam = take((size_t)p->Kpad * 4);
     // owner-private panels P[slice, :], W[slice, :]: shared memory unless that crowds out the rest
     const size_t panel = (size_t)p->Ns * p->Kpad * 4;
@@ -341,10 +341,12 @@ int make_fused_plan(pca_ctx* c, int want) {
   // LL exchange buffers + status word: one contiguous region, zeroed before every launch
   c->ws_off_xchg = off;
   c->ws_off_qx = take((size_t)2 * p.Gs * p.G * p.Ns * 8);
-  c->ws_off_sbx = take((size_t)2 * p.G * (2 + p.Kpad) * 8);
+  c->ws_off_sbx = take((size_t)2 * p.G * (4 + p.Kpad) * 8);
   c->ws_off_ax = take((size_t)2 * p.Gs * p.Kpad * 8);
   c->ws_off_px = take((size_t)2 * p.Gs * p.Ns * 8);
   c->ws_off_nx = take((size_t)2 * p.Gs * 2 * 8);
+  c->ws_off_pfx = take((size_t)2 * p.Gs * p.Ns * 8);
+  c->ws_off_nfx = take((size_t)2 * p.Gs * 2 * 8);
   c->ws_off_pown = take(p.cache_pw ? 0 : (size_t)p.Gs * p.Ns * p.Kpad * 4);
   c->ws_off_wown = take(p.cache_pw ? 0 : (size_t)p.Gs * p.Ns * p.Kpad * 4);
   c->ws_off_status = take(256);
@@ -357,7 +359,6 @@ int make_fused_plan(pca_ctx* c, int want) {
   c->fprm = p;
   c->fvariant = var;
   c->ffn = fn;
-  c->fprm.l2_tail = c->opt_l2_tail >= 0 ? c->opt_l2_tail : 100;       // measured: 0 .. 260 permille within 1-2 % of each other
   c->ring_rows = tma_rb;
   c->smem_bytes = smem;
   c->path = path;
@@ -415,7 +416,7 @@ int make_reg_plan(pca_ctx* c) {
     p.off_wc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
     p.off_x = -1;
     if (G == 1) {                                                     // one CTA: exchange buffers in shared memory if they fit
-      const size_t xwords = (size_t)4 * ldr + 4 * (1 + p.Kpad / 2) + 4 * (2 + p.Kpad) + 4 * (p.Kpad / 2) + 2 * (Gs * 2 + 4);
+      const size_t xwords = (size_t)6 * ldr + 4 * (1 + p.Kpad / 2) + 4 * (2 + p.Kpad) + 4 * (p.Kpad / 2) + 2 * (Gs * 2 + 6) + 2 * (Gs * 2);
       if (off + xwords * 8 <= (size_t)c->smem_optin) p.off_x = take(xwords * 8);
     }
     return off;
@@ -451,7 +452,9 @@ int make_reg_plan(pca_ctx* c) {
   c->ws_off_bx = take((size_t)2 * (2 + p.Kpad) * 2 * 8);
   c->ws_off_ax = take((size_t)2 * p.Gs * p.Kpad * 8);
   c->ws_off_px = take((size_t)2 * ldr * 8);
-  c->ws_off_nx = take((size_t)2 * p.Gs * 8 * 8);
+  c->ws_off_nx = take((size_t)2 * (p.Gs * 2 + 6) * 8);
+  c->ws_off_pfx = take((size_t)2 * ldr * 8);
+  c->ws_off_nfx = take((size_t)2 * p.Gs * 2 * 8);
   c->ws_off_status = take(256);
   c->ws_xchg_bytes = off - c->ws_off_xchg;
   c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1) * 8 : 0);
@@ -667,10 +670,6 @@ int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
       if (value < 0 || value > 8) return PCA_EINVAL;
       c->opt_ring_slots = (int)value;
       break;
-    case PCA_OPT_L2_TAIL:
-      if (value < -1 || value > 1000) return PCA_EINVAL;
-      c->opt_l2_tail = (int)value;
-      break;
     default:
       return PCA_EINVAL;
   }
@@ -807,6 +806,8 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     p.Ax = reinterpret_cast<u64*>(ws + c->ws_off_ax);
     p.Px = reinterpret_cast<u64*>(ws + c->ws_off_px);
     p.Nx = reinterpret_cast<u64*>(ws + c->ws_off_nx);
+    p.Pfx = reinterpret_cast<u64*>(ws + c->ws_off_pfx);
+    p.Nfx = reinterpret_cast<u64*>(ws + c->ws_off_nfx);
     p.status = reinterpret_cast<unsigned*>(ws + c->ws_off_status);
     p.trace = reinterpret_cast<unsigned long long*>(ws + c->ws_off_trace);
     PCA_CUDA(c, cudaMemsetAsync(ws + c->ws_off_xchg, 0, c->ws_xchg_bytes, st));   // sequence numbers start at 0
@@ -833,6 +834,8 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     p.Ax = reinterpret_cast<u64*>(ws + c->ws_off_ax);
     p.Px = reinterpret_cast<u64*>(ws + c->ws_off_px);
     p.Nx = reinterpret_cast<u64*>(ws + c->ws_off_nx);
+    p.Pfx = reinterpret_cast<u64*>(ws + c->ws_off_pfx);
+    p.Nfx = reinterpret_cast<u64*>(ws + c->ws_off_nfx);
     p.Pown = reinterpret_cast<float*>(ws + c->ws_off_pown);
     p.Wown = reinterpret_cast<float*>(ws + c->ws_off_wown);
     p.status = reinterpret_cast<unsigned*>(ws + c->ws_off_status);

@@ -63,10 +63,13 @@ struct FusedParams {
   int Kpad;
   // LL exchange buffers: 8-byte words {payload, seq}, double-buffered by sweep parity (see "LL exchange" below)
   unsigned long long* Qx;   // [2][Gs][G][Ns]   partial raw loads, grouped by slice owner
-  unsigned long long* SBx;  // [2][G][2 + Kpad] words 0-1: partial |t~|^2 (fp64 bits); word 2+j: partial B[j]
+  unsigned long long* SBx;  // [2][G][4 + Kpad] words 0-1: partial |t~|^2 (fp64 bits); words 2-3: this CTA's share of |A|^2
+                            //                  (fp64 bits; deferred loads-side Gram-Schmidt, see the kernel); word 4+j: partial B[j]
   unsigned long long* Ax;   // [2][Gs][Kpad]    partial A
   unsigned long long* Px;   // [2][Gs*Ns]       p^ (orthogonalised, not normalised)
-  unsigned long long* Nx;   // [2][Gs][2]       partial |p^|^2 (fp64 bits)
+  unsigned long long* Nx;   // [2][Gs][2]       partial |p~|^2 (fp64 bits)
+  unsigned long long* Pfx;  // [2][Gs*Ns]       final orthogonalised loads p^ of a component (buffer = component parity)
+  unsigned long long* Nfx;  // [2][Gs][2]       partial |p^|^2 of the final loads
   float* Pown;              // [Gs][Ns][Kpad]   owner-private panels P[slice, :], W[slice, :] (W = R^T V) when
   float* Wown;              //                  they do not fit in shared memory (cache_pw == 0)
   int cache_pw;
@@ -78,7 +81,6 @@ struct FusedParams {
   // TMA-staged streaming kernel (pca_tma.cuh, path 7)
   float* Vrm;                 // [M][Kpad] row-major copy of the unit score vectors (helper warps: B-partials during the sweep)
   int SG;                     // ring slots per row group
-  int l2_tail;                // permille of a sweep's batches fetched with L2 evict_last (PCA_OPT_L2_TAIL)
   int off_ring, off_mbar, off_hb, off_cmd, off_prog;
   // shared-memory carve-up (byte offsets)
   int off_p, off_pdef, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_lam, off_pc, off_wc,
@@ -86,6 +88,13 @@ struct FusedParams {
 };
 
 constexpr int kRB = 4;   // rows per batch
+// When may S3 (the loads-side Gram-Schmidt p^ = p~ - P A) be deferred?  Sweeping with p~/|p^| instead of
+// p^/|p^| adds  R P_(k) A / |p^| = V_(k) Bm A / |p^|  to t~ (Bm = matrix of the final coefficient vectors B_j of the finished
+// components: R_(j+1) p_j = V_(j) B_j).  The scores-side projection removes it exactly, but lambda'^2 = |t~|^2 - |B|^2 is a
+// difference: its rounding error grows with |B|^2 / lambda'^2.  The added part is at most |Bm|_F |A| / |p^| long, so a pass
+// defers only if the previous pass measured   |A|^2 |Bm|_F^2 <= kDeferKappa |p~|^2 lambda'^2   (added part <= 10 % of lambda':
+// no visible cancellation); otherwise, and in the first two passes of a component, it takes the paper's order.
+constexpr double kDeferKappa = 1e-2;
 
 // Phase trace (include/pca.h, PCA_OPT_TRACE): thread 0 of CTA 0 appends (phase << 56) | clock64().
 enum { TR_COMPONENT = 1, TR_LOADS_DONE = 2, TR_X1 = 3, TR_TEST = 4, TR_QSLICE = 5, TR_APART = 6, TR_X2 = 7,
@@ -363,7 +372,7 @@ __device__ __forceinline__ void gl_wait2(const u64* p, unsigned seq, u64& a, u64
 struct RegGather {
   const u64* base;
   int stride, hp, npairs, nparts;
-  bool f64_pair0;
+  int f64_pair0;      // the first f64_pair0 pairs hold ONE fp64 value each
   double2* red;       // kThreads entries
   double* out;
 };
@@ -385,7 +394,7 @@ __device__ __forceinline__ void reg_gather_finish(const RegGather& gq, u64 (&x)[
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int hp = gq.hp;
   const int pair = tid & (hp - 1), pslot = tid / hp, pstep = kThreads / hp;
-  const bool f64 = gq.f64_pair0 && pair == 0;
+  const bool f64 = pair < gq.f64_pair0;
   double a0 = 0.0, a1 = 0.0;
   if (pair < gq.npairs) {
 #pragma unroll
@@ -444,7 +453,7 @@ struct LLJob {
   const u64* base;
   double* out;
   int units, nparts, stride;
-  bool f64_unit0;
+  int f64_unit0;      // the first f64_unit0 units hold ONE fp64 value each (words 0-1 of the unit)
 };
 constexpr int kLLParts = 5;                 // parts per lane held in flight (covers 160 CTAs in one round)
 
@@ -464,7 +473,7 @@ __device__ __forceinline__ void ll_reduce_unit(const LLJob& jb, int u, unsigned 
       const int bq = b0 + 32 * i;
       if (bq < jb.nparts) {
         ll_wait2(jb.base + (size_t)bq * jb.stride + 2 * u, seq, x[i], y[i], status);
-        if (jb.f64_unit0 && u == 0) a0 += ll_d(x[i], y[i]);
+        if (u < jb.f64_unit0) a0 += ll_d(x[i], y[i]);
         else { a0 += (double)ll_f(x[i]); a1 += (double)ll_f(y[i]); }
       }
     }
@@ -526,11 +535,11 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
   float* qs = reinterpret_cast<float*>(smem + prm.off_qs);        // NG x ldr group partials
   float* red_s = reinterpret_cast<float*>(smem + prm.off_red);    // 2 x kWarps x kRB
   double* sgrp = reinterpret_cast<double*>(smem + prm.off_sgrp);  // NG
-  double* sb_s = reinterpret_cast<double*>(smem + prm.off_B);     // 2 + Kpad: |t~|^2, -, B
-  double* B_s = sb_s + 2;
+  double* sb_s = reinterpret_cast<double*>(smem + prm.off_B);     // 4 + Kpad: |t~|^2, -, |A|^2, -, B
+  double* B_s = sb_s + 4;
   double* A_s = reinterpret_cast<double*>(smem + prm.off_A);      // Kpad
   double* scr = reinterpret_cast<double*>(smem + prm.off_scr);    // kThreads
-  double* ctl_s = scr + kThreads - 4;                             // lambda', decision, 1/|p^| of the current pass
+  double* ctl_s = scr + kThreads - 8;                             // lambda', decision, 1/|p^| of the current pass
   double* praw_s = reinterpret_cast<double*>(smem + prm.off_praw);// Ns: p~ / p^ slice of this owner
   float* lam_s = reinterpret_cast<float*>(smem + prm.off_lam);    // Kpad
   float* slab = reinterpret_cast<float*>(smem + prm.off_slab);    // resident: Mb x ldr
@@ -542,7 +551,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
   const int N = prm.N, K = prm.K, G = prm.G, ldr = prm.ldr, Kpad = prm.Kpad, Ns = prm.Ns, Gs = prm.Gs;
   const int NG = kThreads / prm.GT;
   const int npx = Gs * Ns;                                 // exchanged length of p (>= N)
-  const int SBw = 2 + Kpad;
+  const int SBw = 4 + Kpad;
   const bool gs = prm.algo == 1;
   const long long m0 = (long long)b * prm.Mb;
   const int mb = (int)max(0LL, min((long long)prm.Mb, M - m0));
@@ -550,12 +559,15 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
   const int ns = max(0, min(Ns, N - n0));
   const bool owner = ns > 0;
   unsigned seq = 0;                                        // sweep number; parity selects the exchange buffers
-  unsigned e1 = 0, e2 = 0, e3 = 0;                         // expected values of the three arrival counters
+  unsigned e1 = 0, e2 = 0, e3 = 0, e4 = 0;                 // expected values of the arrival counters
   unsigned* const cnt1 = prm.cnt;
   unsigned* const cnt2 = prm.cnt + 64;
   unsigned* const cnt3 = prm.cnt + 128;
+  unsigned* const cnt4 = prm.cnt + 192;
+  double* praw2_s = praw_s + Ns;                           // second slice buffer (final p^ of a component)
   unsigned* status = prm.status;
   int tn = 0;                                              // trace records written (thread 0 of CTA 0)
+  double bf2 = 0.0;                                        // sum over the finished components of |B_j|^2 (see kDeferKappa)
 
   float* Rb = prm.Rrm + (size_t)m0 * ldr;
   float* Tb = prm.T + m0;
@@ -610,6 +622,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
     int it = 0;
     bool degenerate = false;
     bool first = true;
+    float inv_pn = 0.f;                                      // 1/|p~| (1/|p^|) of the pass in flight
+    bool deferred = false;                                   // the loads of the pass in flight are p~ (S3 deferred), not p^
     for (;;) {
       const unsigned par = seq & 1u;
       // ---- hop 1: |t~|^2 and B (every CTA), raw loads slice (owners) ----
@@ -619,8 +633,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         LLJob jq, jsb;
         jq.base = prm.Qx + ((size_t)par * Gs + b) * G * Ns; jq.out = praw_s; jq.units = owner ? (Ns >> 1) : 0;
         jq.nparts = G; jq.stride = Ns; jq.f64_unit0 = false;
-        jsb.base = prm.SBx + (size_t)par * G * SBw; jsb.out = sb_s; jsb.units = 1 + ((gsk && !first) ? ((k + 1) >> 1) : 0);
-        jsb.nparts = G; jsb.stride = SBw; jsb.f64_unit0 = true;
+        jsb.base = prm.SBx + (size_t)par * G * SBw; jsb.out = sb_s; jsb.units = (gsk && !first) ? 2 + ((k + 1) >> 1) : 1;
+        jsb.nparts = G; jsb.stride = SBw; jsb.f64_unit0 = 2;
         if (jsb.units <= 16) {
           ll_reduce2(jsb, jq, seq, status);
         } else {
@@ -629,7 +643,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           RegGather gsb;
           int hs = 32;
           while (hs < jsb.units) hs <<= 1;
-          gsb.base = jsb.base; gsb.stride = SBw; gsb.hp = hs; gsb.npairs = jsb.units; gsb.nparts = G; gsb.f64_pair0 = true;
+          gsb.base = jsb.base; gsb.stride = SBw; gsb.hp = hs; gsb.npairs = jsb.units; gsb.nparts = G; gsb.f64_pair0 = 2;
           gsb.red = reinterpret_cast<double2*>(qs); gsb.out = sb_s;
           u64 sx[8], sy[8];
           reg_gather_issue<8>(gsb, sx, sy);
@@ -656,7 +670,23 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
             for (int j = lane; j < k; j += 32) bb += B_s[j] * B_s[j];
             bb = warp_sum(bb);
           }
-          const double l2 = s - bb;                                           // |t~ - V B|^2, V orthonormal
+          double l2 = s - bb;                                                 // |t~ - V B|^2, V orthonormal
+          double rho = 1.0;
+          if (gsk) {
+            const double pn2 = ctl_s[3], a2 = sb_s[2];
+            if (deferred) {
+              // deferred loads-side Gram-Schmidt (see "S3" below): the sweep ran with p~/|p~| instead of p^/|p^|,
+              // |p^|^2 = |p~|^2 - |A|^2 (P orthonormal), so every product of the sweep is short of the paper's by
+              // rho = |p~|/|p^|
+              const double d2 = pn2 - a2;
+              if (!(d2 > 0.0)) l2 = 0.0;
+              else rho = sqrt(pn2 / d2);
+              l2 *= rho * rho;
+            }
+            // the NEXT pass defers S3 only if that is harmless (same decision on every CTA): see kDeferKappa
+            if (lane == 0) reinterpret_cast<int*>(ctl_s + 4)[0] = (a2 * bf2 <= kDeferKappa * pn2 * lam * lam) ? 1 : 0;
+          }
+          if (lane == 0) ctl_s[2] = rho;
           if (!(l2 > 0.0)) st = 2;                                            // reading C7
           else {
             ln = sqrt(l2);                                                    // S7
@@ -698,16 +728,27 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       if (done) break;
       trace_mark(prm, tn, TR_QSLICE);
 
-      if (gsk && owner) {
-        if (tid == 0) hop_arrive(cnt2);                                       // A-partials of this pass are out
-        trace_mark(prm, tn, TR_APART);
-        e2 += (unsigned)Gs;
+      // ---- S3, deferred.  The paper orthogonalises the loads first, p^ = p~ - P_(k) A, and multiplies
+      // then, t~ = R p^.  R P_(k) lies in span V_(k) (deflation: R_(j+1) p_j = t~_j - t_j = V_(j) B_j, and later deflations
+      // add multiples of v_i), and the scores-side projection t = t~ - V_(k) V_(k)^T t~ removes that
+      // span, so R p~ and R p^ give the SAME t: the sweep can start from p~ without waiting for A = sum of the owners'
+      // partials (one dependent cross-CTA hop less per pass).  What the iteration needs from A is |p^|^2 = |p~|^2 - |A|^2
+      // (lambda' scales with 1/|p^|); it travels with the NEXT exchange.  p^ itself is formed once, when the component has
+      // converged ("final loads" below).  (The two-sweep kernel keeps the paper's literal order.)
+      // Deferring costs accuracy when A is NOT small (the first pass of a component starts from a raw column; fixed-pass
+      // runs never converge): t~ then carries a large component in span V_(k) and lambda'^2 = |t~|^2 - |B|^2 cancels.  So the
+      // first two passes of a component, and every pass for which the bound of kDeferKappa fails, take the paper's order.
+      const bool defer_now = gsk && !first && reinterpret_cast<const int*>(ctl_s + 4)[0] != 0;
+      if (gsk && owner && tid == 0) hop_arrive(cnt2);                         // A-partials of this pass are out
+      trace_mark(prm, tn, TR_APART);
+      if (gsk) e2 += (unsigned)Gs;
+      if (gsk && owner && !defer_now) {
         hop_wait(cnt2, e2, status);
         // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
         if (k <= 30) {
           LLJob ja, jn;
           ja.base = prm.Ax + (size_t)par * Gs * Kpad; ja.out = A_s; ja.units = (k + 1) >> 1; ja.nparts = Gs; ja.stride = Kpad;
-          ja.f64_unit0 = false;
+          ja.f64_unit0 = 0;
           jn = ja; jn.units = 0;
           ll_reduce2(ja, jn, seq, status);
         } else {
@@ -716,7 +757,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           int ha = 32;
           while (ha < ua) ha <<= 1;
           ga.base = prm.Ax + (size_t)par * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
-          ga.f64_pair0 = false; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
+          ga.f64_pair0 = 0; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
           u64 ax8[8], ay8[8];
           reg_gather_issue<8>(ga, ax8, ay8);
           reg_gather_finish<8>(ga, ax8, ay8, seq, status);
@@ -728,7 +769,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         slice_correct(praw_s, Pc, A_s, ns, k, Kpad);
         __syncthreads();
       }
-      // ---- publish the p^ slice and its squared norm (S4, first half) ----
+      deferred = defer_now;
+      // ---- publish the p~ slice and its squared norm (S4, first half) ----
       if (owner && w == 0) {
         double q2 = 0.0;
         for (int u = lane; 2 * u < Ns; u += 32) {
@@ -752,7 +794,27 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         jn.base = prm.Nx + (size_t)par * Gs * 2; jn.out = scr; jn.units = 1; jn.nparts = Gs; jn.stride = 2; jn.f64_unit0 = true;
         ll_reduce_unit(jn, 0, seq, status);
         __syncwarp();
-        if (lane == 0) reinterpret_cast<float*>(ctl_s + 2)[0] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+        if (lane == 0) {
+          ctl_s[3] = scr[0];                                                  // |p~|^2
+          reinterpret_cast<float*>(ctl_s + 1)[1] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+        }
+      }
+      if (gsk && w == kWarps - 2) {
+        // this CTA's share of |A|^2: the entries A[2u], A[2u+1] of its units u = b, b + G, ... summed over the owners'
+        // partials (fixed order); published with |t~|^2 after the sweep, summed over the CTAs at the next hop 1
+        double a2 = 0.0;
+        LLJob ja;
+        ja.base = prm.Ax + (size_t)par * Gs * Kpad; ja.out = scr + 8; ja.nparts = Gs; ja.stride = Kpad; ja.f64_unit0 = 0;
+        ja.units = (k + 1) >> 1;
+        double* ao = scr + 8;                                                  // (scr[0..] belongs to the norm warp)
+        for (int u = b; u < ja.units; u += G) {
+          ja.out = ao - 2 * u;                                                // the unit's two sums land in ao[0], ao[1]
+          ll_reduce_unit(ja, u, seq, status);
+          __syncwarp();
+          a2 += ao[0] * ao[0] + ao[1] * ao[1];
+          __syncwarp();
+        }
+        if (lane == 0) scr[4] = a2;
       }
       {
         const u64* px = prm.Px + (size_t)par * npx;
@@ -776,7 +838,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       }
       __syncthreads();
       trace_mark(prm, tn, TR_X3);
-      const float inv_pn = reinterpret_cast<const float*>(ctl_s + 2)[0];      // p = p^/|p^|
+      inv_pn = reinterpret_cast<const float*>(ctl_s + 1)[1];                  // p = p~/|p~| (see S3 above)
+      const double a2mine = gsk ? scr[4] : 0.0;
       if (!(inv_pn > 0.f)) { degenerate = true; break; }                      // reading C7
       for (int n = tid; n < npx; n += kThreads) p_s[n] *= inv_pn;             // each thread rescales what it wrote
       __syncthreads();
@@ -797,7 +860,10 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           double a = 0.0;
           for (int g = 0; g < NG; ++g) a += sgrp[g];
           ll_st2d(sbx, a, seq);
+          if (gsk) ll_st2d(sbx + 2, a2mine, seq);
         }
+        __syncthreads();   // (measured: without this barrier the B-partial loop below runs 2-6 x slower -- warp 0 enters it
+                           //  diverged from the tid == 0 block above and its full-mask shuffles pay for it every iteration)
         if (gsk) {                                                            // S6: B-partials V^T t~
           // the CTA's rows of the first Ksm unit score vectors are cached in shared memory (Vc, column-major), the rest
           // comes from T in global memory (L2)
@@ -822,7 +888,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
               }
             }
             const double s0 = warp_sum((double)a0), s1 = warp_sum((double)a1);
-            if (lane == 0) ll_st2(sbx + 2 + j0, ll_wordf((float)s0, seq), ll_wordf((float)s1, seq));
+            if (lane == 0) ll_st2(sbx + 4 + j0, ll_wordf((float)s0, seq), ll_wordf((float)s1, seq));
           }
         }
         __syncthreads();                                                      // all LL stores of this CTA are issued
@@ -831,6 +897,86 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       }
     }
 
+    if (!degenerate && gsk && deferred) {
+      // ---- final loads (once per component, if the pass that converged had S3 deferred): p^ = p~ - P_(k) A (S3) of the pass that converged,
+      //      p = p^/|p^| (S4).  p_s holds p~/|p~|, the owners' A-partials of that pass are in Ax. ----
+      const unsigned apar = (seq - 1u) & 1u, aseq = seq - 1u;
+      const unsigned fpar = (unsigned)k & 1u, ftag = (unsigned)k + 1u;
+      if (owner) {
+        if (k <= 30) {
+          LLJob ja, jn;
+          ja.base = prm.Ax + (size_t)apar * Gs * Kpad; ja.out = A_s; ja.units = (k + 1) >> 1; ja.nparts = Gs; ja.stride = Kpad;
+          ja.f64_unit0 = 0;
+          jn = ja; jn.units = 0;
+          ll_reduce2(ja, jn, aseq, status);
+        } else {
+          RegGather ga;
+          const int ua = (k + 1) >> 1;
+          int ha = 32;
+          while (ha < ua) ha <<= 1;
+          ga.base = prm.Ax + (size_t)apar * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
+          ga.f64_pair0 = 0; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
+          u64 ax8[8], ay8[8];
+          reg_gather_issue<8>(ga, ax8, ay8);
+          reg_gather_finish<8>(ga, ax8, ay8, aseq, status);
+          __syncthreads();
+          reg_gather_store(ga);
+        }
+        __syncthreads();
+        for (int i = tid; i < Ns; i += kThreads) praw2_s[i] = (i < ns) ? (double)p_s[n0 + i] : 0.0;
+        for (int j = tid; j < k; j += kThreads) A_s[j] *= (double)inv_pn;   // A of the scaled vector p~/|p~|
+        __syncthreads();
+        slice_correct(praw2_s, Pc, A_s, ns, k, Kpad);
+        __syncthreads();
+        if (w == 0) {
+          double q2 = 0.0;
+          for (int u = lane; 2 * u < Ns; u += 32) {
+            const float v0 = (2 * u < ns) ? (float)praw2_s[2 * u] : 0.f;
+            const float v1 = (2 * u + 1 < ns) ? (float)praw2_s[2 * u + 1] : 0.f;
+            ll_st2(prm.Pfx + (size_t)fpar * npx + n0 + 2 * u, ll_wordf(v0, ftag), ll_wordf(v1, ftag));
+            q2 += (double)v0 * (double)v0 + (double)v1 * (double)v1;
+          }
+          q2 = warp_sum(q2);
+          if (lane == 0) {
+            ll_st2d(prm.Nfx + ((size_t)fpar * Gs + b) * 2, q2, ftag);
+            hop_arrive(cnt4);
+          }
+        }
+      }
+      e4 += (unsigned)Gs;
+      hop_wait(cnt4, e4, status);
+      if (w == kWarps - 1) {
+        LLJob jn;
+        jn.base = prm.Nfx + (size_t)fpar * Gs * 2; jn.out = scr; jn.units = 1; jn.nparts = Gs; jn.stride = 2; jn.f64_unit0 = 1;
+        ll_reduce_unit(jn, 0, ftag, status);
+        __syncwarp();
+        if (lane == 0) reinterpret_cast<float*>(ctl_s + 1)[1] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+      }
+      {
+        const u64* px = prm.Pfx + (size_t)fpar * npx;
+        for (int u0 = tid; 2 * u0 < npx; u0 += kThreads * 4) {
+          u64 x[4], y[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int u = u0 + i * kThreads;
+            x[i] = 0; y[i] = 0;
+            if (2 * u < npx) ll_ld2(px + 2 * u, x[i], y[i]);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int u = u0 + i * kThreads;
+            if (2 * u < npx) {
+              ll_wait2(px + 2 * u, ftag, x[i], y[i], status);
+              *reinterpret_cast<float2*>(p_s + 2 * u) = make_float2(ll_f(x[i]), ll_f(y[i]));
+            }
+          }
+        }
+      }
+      __syncthreads();
+      const float inv_f = reinterpret_cast<const float*>(ctl_s + 1)[1];
+      for (int n = tid; n < npx; n += kThreads) p_s[n] *= inv_f;
+      __syncthreads();
+    }
     // ---- component done ----
     if (degenerate) {
       for (int i = tid; i < mb; i += kThreads) {
@@ -845,13 +991,20 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
     } else {
       const float lamf = (float)lam_new;
       const float inv = (float)(1.0 / lam_new);
+      const double rho = (gsk && deferred) ? ctl_s[2] : 1.0;                               // products of the last sweep are short by rho (S3)
+      const float rhof = (float)rho;
+      if (gsk) {                                                              // |B_k|^2 of the finished component (every thread: uniform)
+        double bb = 0.0;
+        for (int j = 0; j < k; ++j) bb += B_s[j] * B_s[j];
+        bf2 += bb * rho * rho;
+      }
       // t = t~ - V_(k) B;  GS-PCA: v = t/lambda'
       for (int i = tid; i < mb; i += kThreads) {
         float t = ttil_s[i];
         if (gsk) {
           float corr = 0.f;
           for (int j = 0; j < k; ++j) corr = fmaf(Tb[(size_t)j * M + i], (float)B_s[j], corr);
-          t -= corr;
+          t = (t - corr) * rhof;
         }
         d_s[i] = t;                                                           // R -= lambda v p^T  /  R -= t p^T
         Tb[(size_t)k * M + i] = (gs || prm.out_svd) ? t * inv : t;
@@ -862,7 +1015,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
         prm.P[(size_t)k * N + n0 + tid] = pk;
         Pc[(size_t)tid * Kpad + k] = pk;
         if (gs && k + 1 < K)                                                  // W_k = R_(k+1)^T v_k
-          Wc[(size_t)tid * Kpad + k] = (float)(praw_s[tid] / lam_new - lam_new * (double)pk);
+          Wc[(size_t)tid * Kpad + k] = (float)(praw_s[tid] * rho / lam_new - lam_new * (double)pk);
       }
       for (int n = tid; n < ldr; n += kThreads) pdef_s[n] = (n < npx) ? p_s[n] : 0.f;
       if (b == 0 && tid == 0) { prm.lambda[k] = lamf; prm.iters[k] = it; }

@@ -54,8 +54,10 @@ struct RegParams {
   unsigned long long* Bx;   // [2][2 + Kpad][2]    two-level: entry e as fp64 bits (entry 0 = |t~|^2, entry 2+j = B[j])
   unsigned long long* Ax;   // [2][Gs*Kpad]        partial A (fp32) of each owner; k <= 64: unit-major [Kpad/2][Gs][2] (a warp per unit,
                             //                     lanes over the owners), else owner-major [Gs][Kpad] (lanes over the units, owners in turn)
-  unsigned long long* Px;   // [2][ldr]            p^ (orthogonalised, not normalised)
-  unsigned long long* Nx;   // [2][Gs*2 + 4]       per owner: partial |p^|^2 (fp64, 2 words); then {decision, -, lambda' (fp64)}
+  unsigned long long* Px;   // [2][ldr]            p~ (loads before the loads-side projection, not normalised)
+  unsigned long long* Nx;   // [2][Gs*2 + 6]       per owner: partial |p~|^2 (fp64, 2 words); then {decision, -, lambda' (fp64), rho (fp64)}
+  unsigned long long* Pfx;  // [2][ldr]            final orthogonalised loads p^ of a component (buffer = component parity)
+  unsigned long long* Nfx;  // [2][Gs*2]           per owner: partial |p^|^2 of the final loads
   unsigned* status;         // [0] != 0: an exchange wait gave up
   unsigned long long* trace;
   int trace_cap;
@@ -386,6 +388,28 @@ __device__ __forceinline__ void reg_publish_a(const float* Pc, int KP, const dou
     gl_st2(ax + (size_t)(j >> 1) * ustride, ll_wordf((float)a, seq), ll_wordf(j + 1 < k ? (float)nb : 0.f, seq));
 }
 
+// A = sum over the owners of their partials, published with tag `tag` in parity buffer `par`; all threads
+// of the CTA; the caller synchronises before reading A_s.  scratch: kThreads double2 (k > 64 only).
+__device__ __forceinline__ void reg_gather_a(const RegParams& prm, const u64* Ax, unsigned par, unsigned tag, int k, float* scratch,
+                                             double* A_s, unsigned* status) {
+  const int Gs = prm.Gs, Kpad = prm.Kpad;
+  if (k <= 64) {                                                      // few units: a warp per unit, lanes over the owners
+    reg_ll_reduce_all(Ax + (size_t)par * Gs * Kpad, 2, Gs * 2, Gs, (k + 1) >> 1, tag, status, A_s);
+  } else {                                                            // many units: lanes over the units (coalesced), owners in turn
+    RegGather ga;
+    const int ua = (k + 1) >> 1;
+    int ha = 1;
+    while (ha < ua) ha <<= 1;
+    ga.base = Ax + (size_t)par * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
+    ga.f64_pair0 = 0; ga.red = reinterpret_cast<double2*>(scratch); ga.out = A_s;
+    u64 ax8[8], ay8[8];
+    reg_gather_issue<8>(ga, ax8, ay8);
+    reg_gather_finish<8>(ga, ax8, ay8, tag, status);
+    __syncthreads();
+    reg_gather_store(ga);
+  }
+}
+
 // ------------------------------------------------------------------------------------ the kernel
 template <int GT, int NV, int RPT>
 __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams prm) {
@@ -413,12 +437,13 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
   const int b = blockIdx.x;
   const long long M = prm.M;
   const int N = prm.N, K = prm.K, G = prm.G, ldr = prm.ldr, Kpad = prm.Kpad, Ns = prm.Ns, Gs = prm.Gs;
-  u64 *Qx = prm.Qx, *SBx = prm.SBx, *Bx = prm.Bx, *Ax = prm.Ax, *Px = prm.Px, *Nx = prm.Nx;
+  u64 *Qx = prm.Qx, *SBx = prm.SBx, *Bx = prm.Bx, *Ax = prm.Ax, *Px = prm.Px, *Nx = prm.Nx, *Pfx = prm.Pfx, *Nfx = prm.Nfx;
+  const int NXW = Gs * 2 + 6;                                      // words per parity buffer of Nx
   if (prm.off_x >= 0) {                                            // one CTA: exchange through shared memory
     u64* xb = reinterpret_cast<u64*>(smem + prm.off_x);
     Qx = xb; SBx = Qx + 2 * (size_t)ldr; Bx = SBx + 4 * (1 + (Kpad >> 1)); Ax = Bx + 4 * (2 + Kpad); Px = Ax + 4 * (Kpad >> 1);
-    Nx = Px + 2 * (size_t)ldr;
-    const int nw = (int)(Nx + 2 * (Gs * 2 + 4) - xb);
+    Nx = Px + 2 * (size_t)ldr; Pfx = Nx + 2 * NXW; Nfx = Pfx + 2 * (size_t)ldr;
+    const int nw = (int)(Nfx + 2 * (Gs * 2) - xb);
     for (int i = tid; i < nw; i += kThreads) xb[i] = 0ULL;         // sequence numbers start at 0
   }
   double* pt_s = praw_s + Ns;                                      // Ns: R^T t slice (p~ before the loads-side projection), for W
@@ -433,6 +458,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
   unsigned seq = 0;
   unsigned* status = prm.status;
   int tn = 0;
+  double bf2 = 0.0;                                                // sum over the finished components of |B_j|^2 (kDeferKappa)
   float* Rb = prm.Rrm + (size_t)m0 * ldr;
   float* Tb = prm.T + m0;
 
@@ -466,6 +492,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
     reg_trace(prm, tn, TR_LOADS_DONE);
 
     double lam = 0.0, lam2 = 0.0, lam_new = 0.0;                    // lambda of the previous pass, of the one before, of this one
+    float rhof = 1.f;                                               // |p~|/|p^| of the pass that converged (S3, deferred)
+    bool deferred = false;                                          // the loads of the pass in flight are p~, not p^
     int it = 0;
     bool degenerate = false, first = true;
     float pscale = 0.f;
@@ -508,6 +536,19 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           }
         }
         __syncthreads();                                                      // qs (group partials of the sweep) is free
+        if (with_b) {
+          // deferred loads-side Gram-Schmidt (see "S3, deferred" below): every owner sums the A-partials the owners published
+          // one pass ago (they have been there for a whole sweep): |p^|^2 = |p~|^2 - |A|^2 for owner 0's test, and the
+          // decision whether the next pass may defer again
+          reg_gather_a(prm, Ax, (seq - 1u) & 1u, seq - 1u, k, qs, A_s, status);
+          __syncthreads();
+          if (w == 0) {
+            double a2 = 0.0;
+            for (int j = lane; j < k; j += 32) a2 += A_s[j] * A_s[j];
+            a2 = warp_sum(a2);
+            if (lane == 0) ctl_s[6] = a2;
+          }
+        }
         if ((Ns >> 1) <= kThreads) {
           u64 qx[5], qy[5];
           reg_gather_issue<5>(gq, qx, qy);
@@ -559,6 +600,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         __syncthreads();
         reg_trace(prm, tn, TR_X1);
         // S7/S8 by warp 0 of owner 0 (then it joins the others);  p~ = q - W B on the owner's slice (needs only B)
+        if (w == 0 && lane == 0 && (b != 0 || first)) ctl_s[7] = 1.0;
         if (w == 0 && b != 0 && lane == 0) { ctl_s[0] = 0.0; reinterpret_cast<int*>(ctl_s + 1)[0] = 0; }
         if (w == 0 && b == 0) {
           const double s = sb_s[0];
@@ -572,7 +614,15 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
               for (int j = lane; j < k; j += 32) bb += B_s[j] * B_s[j];
               bb = warp_sum(bb);
             }
-            const double l2 = s - bb;                                         // |t~ - V B|^2, V orthonormal
+            double l2 = s - bb;                                               // |t~ - V B|^2, V orthonormal
+            double rho = 1.0;
+            if (gsk && deferred) {                                            // |p^|^2 = |p~|^2 - |A|^2 (P orthonormal)
+              const double pn2 = ctl_s[5], d2 = pn2 - ctl_s[6];
+              if (!(d2 > 0.0)) l2 = 0.0;
+              else rho = sqrt(pn2 / d2);
+              l2 *= rho * rho;
+            }
+            if (lane == 0) ctl_s[7] = rho;
             if (!(l2 > 0.0)) st = 2;                                          // reading C7
             else {
               ln = sqrt(l2);                                                  // S7
@@ -589,35 +639,30 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         // S3: a_S[j] = sum_{n in S} P[n,j] p~[n]
         if (gs)
           for (int i2 = tid; i2 < Ns; i2 += kThreads) pt_s[i2] = praw_s[i2];
-        if (gsk) {
-          if (k <= 64) reg_publish_a(Pc, KV, praw_s, Ax + (size_t)par * Gs * Kpad + (size_t)b * 2, Gs * 2, ns, k, seq);
-          else reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * Gs + b) * Kpad, 2, ns, k, seq);
-        }
         const int st = reinterpret_cast<const int*>(ctl_s + 1)[0];
         reg_trace(prm, tn, TR_TEST);
-        if (gsk) {                                                            // (also on the pass that reports "done": only owner 0 knows)
+        // ---- S3, deferred.  The paper orthogonalises the loads first, p^ = p~ - P_(k) A, and multiplies then,
+        // t~ = R p^.  R P_(k) lies in span V_(k) (deflation: R_(j+1) p_j = t~_j - t_j = V_(j) B_j, later deflations add multiples
+        // of v_i), and the scores-side projection t = t~ - V_(k) V_(k)^T t~ removes that span, so R p~ and R p^
+        // give the SAME t: the sweep starts from p~ without waiting for A = sum of the owners' partials (one dependent cross-CTA
+        // hop less per pass).  The iteration needs |p^|^2 = |p~|^2 - |A|^2 (owner 0, at the next test); p^ itself is formed once,
+        // when the component has converged ("final loads" below).  (The two-sweep kernel keeps the paper's literal order.)
+        // Deferring costs accuracy when A is NOT small (the first pass of a component starts from a raw column; fixed-pass runs
+        // never converge): t~ then carries a large component in span V_(k) and lambda'^2 = |t~|^2 - |B|^2 cancels.  So the first
+        // two passes of a component, and every pass for which the bound of kDeferKappa (pca_fused.cuh) fails, take the paper's
+        // order (hop 2).  Every owner takes the same decision from the same numbers.
+        const bool defer_now = with_b && ctl_s[6] * bf2 <= kDeferKappa * ctl_s[5] * lam * lam;
+        if (gsk && !defer_now) {
+          if (k <= 64) reg_publish_a(Pc, KV, praw_s, Ax + (size_t)par * Gs * Kpad + (size_t)b * 2, Gs * 2, ns, k, seq);
+          else reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * Gs + b) * Kpad, 2, ns, k, seq);
           // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
-          if (k <= 64) {                                                      // few units: a warp per unit, lanes over the owners
-            reg_ll_reduce_all(Ax + (size_t)par * Gs * Kpad, 2, Gs * 2, Gs, (k + 1) >> 1, seq, status, A_s);
-          } else {                                                            // many units: lanes over the units (coalesced), owners in turn
-            RegGather ga;
-            const int ua = (k + 1) >> 1;
-            int ha = 1;
-            while (ha < ua) ha <<= 1;
-            ga.base = Ax + (size_t)par * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
-            ga.f64_pair0 = false; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
-            u64 ax8[8], ay8[8];
-            reg_gather_issue<8>(ga, ax8, ay8);
-            reg_gather_finish<8>(ga, ax8, ay8, seq, status);
-            __syncthreads();
-            reg_gather_store(ga);
-          }
+          reg_gather_a(prm, Ax, par, seq, k, qs, A_s, status);
           __syncthreads();
           reg_trace(prm, tn, TR_X2);
           reg_slice_correct(praw_s, Pc, KV, A_s, ns, k);
           __syncthreads();
         }
-        // ---- publish the p^ slice, its squared norm, the decision and lambda' ----
+        // ---- publish the p~ slice, its squared norm, the decision, lambda' and rho ----
         if (w == 0) {
           double q2 = 0.0;
           for (int u = lane; 2 * u < Ns; u += 32) {
@@ -628,32 +673,39 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           }
           q2 = warp_sum(q2);
           if (lane == 0) {
-            u64* nx = Nx + (size_t)par * (Gs * 2 + 4);
+            u64* nx = Nx + (size_t)par * NXW;
             gl_st2d(nx + (size_t)b * 2, q2, seq);
             if (b == 0) {                                                     // every owner takes the same decision: owner 0 reports it
-              gl_st2(nx + (size_t)Gs * 2, ll_word((unsigned)st, seq), ll_word(0u, seq));
+              gl_st2(nx + (size_t)Gs * 2, ll_word((unsigned)st, seq), ll_word(defer_now ? 1u : 0u, seq));
               gl_st2d(nx + (size_t)Gs * 2 + 2, ctl_s[0], seq);
+              gl_st2d(nx + (size_t)Gs * 2 + 4, ctl_s[7], seq);
             }
           }
         }
         reg_trace(prm, tn, TR_PHAT);
+        // S3, first half, off the critical path: a_S[j] = sum_{n in S} P[n,j] p~[n]
+        if (gsk && defer_now) {
+          if (k <= 64) reg_publish_a(Pc, KV, praw_s, Ax + (size_t)par * Gs * Kpad + (size_t)b * 2, Gs * 2, ns, k, seq);
+          else reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * Gs + b) * Kpad, 2, ns, k, seq);
+        }
       }
       // ---- arrival hint: ONE thread of the CTA polls ONE word (the last owner's norm record) while the others sleep at the
       // barrier; only then does every thread load its words of p^ (each validated by its own sequence number, so the hint
       // orders nothing).  Measured: with all 148 x 512 threads polling the same 8 KB the hop takes 2.9-3.3 us, this way 1.8 us.
       if (tid == (kWarps - 1) * 32) {
-        const u64* nxl = Nx + (size_t)par * (Gs * 2 + 4) + (size_t)(Gs - 1) * 2;
+        const u64* nxl = Nx + (size_t)par * NXW + (size_t)(Gs - 1) * 2;
         u64 x = 0, y = 0;
         gl_wait2(nxl, seq, x, y, status);
       }
       __syncthreads();
       // ---- hop 3 (every CTA): gather p^, |p^|^2, the decision and lambda' ----
       if (w == kWarps - 1) {
-        const u64* nx = Nx + (size_t)par * (Gs * 2 + 4);
+        const u64* nx = Nx + (size_t)par * NXW;
         double nsum = 0.0, lamv = 0.0;
         unsigned stv = 0;
-        u64 x1 = 0, y1 = 0, x2 = 0, y2 = 0;
-        if (lane == 0) { gl_ld2(nx + (size_t)Gs * 2, x1, y1); gl_ld2(nx + (size_t)Gs * 2 + 2, x2, y2); }
+        u64 x1 = 0, y1 = 0, x2 = 0, y2 = 0, x3 = 0, y3 = 0;
+        double rhov = 1.0;
+        if (lane == 0) { gl_ld2(nx + (size_t)Gs * 2, x1, y1); gl_ld2(nx + (size_t)Gs * 2 + 2, x2, y2); gl_ld2(nx + (size_t)Gs * 2 + 4, x3, y3); }
         for (int o = lane; o < Gs; o += 32) {
           u64 x0 = 0, y0 = 0;
           gl_wait2(nx + (size_t)o * 2, seq, x0, y0, status);
@@ -662,14 +714,19 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         if (lane == 0) {
           gl_wait2(nx + (size_t)Gs * 2, seq, x1, y1, status);
           gl_wait2(nx + (size_t)Gs * 2 + 2, seq, x2, y2, status);
+          gl_wait2(nx + (size_t)Gs * 2 + 4, seq, x3, y3, status);
           stv = (unsigned)x1;
+          reinterpret_cast<int*>(ctl_s + 1)[1] = (int)(unsigned)y1;             // the loads just published are p~ (S3 deferred)
           lamv = ll_d(x2, y2);
+          rhov = ll_d(x3, y3);
         }
         nsum = warp_sum(nsum);
         if (lane == 0) {
           reinterpret_cast<float*>(ctl_s + 2)[0] = (nsum > 0.0) ? (float)rsqrt(nsum) : 0.f;
           ctl_s[3] = lamv;
           reinterpret_cast<int*>(ctl_s + 4)[0] = (int)stv;
+          reinterpret_cast<float*>(ctl_s + 4)[1] = (float)rhov;
+          ctl_s[5] = nsum;                                                    // |p~|^2 of the loads the next sweep runs with
         }
       }
       {
@@ -699,10 +756,12 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       if (st3 == 2) { degenerate = true; break; }
       if (!first) {
         lam_new = ctl_s[3];
+        rhof = reinterpret_cast<const float*>(ctl_s + 4)[1];
         if (st3 == 1) break;
         lam2 = lam;
         lam = lam_new;
       }
+      deferred = reinterpret_cast<const int*>(ctl_s + 1)[1] != 0;
       pscale = reinterpret_cast<const float*>(ctl_s + 2)[0];                   // p = p^/|p^|
       if (!(pscale > 0.f)) { degenerate = true; break; }                      // reading C7
       first = false;
@@ -735,6 +794,67 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       __syncthreads();
     } else {
       const unsigned par = seq & 1u;
+      if (gsk && deferred) {
+        // ---- final loads (once per component, if S3 was deferred in the pass that converged): p^ = p~ - P_(k) A (S3) of the pass that converged, then
+        //      p = p^/|p^| (S4).  The p~ of that pass is in p_s, the owners' A-partials in Ax. ----
+        const unsigned fpar = (unsigned)k & 1u, ftag = (unsigned)k + 1u;
+        float* pk_w = p_s + (size_t)((it - 1) & 1) * ldr;
+        if (owner) {
+          reg_gather_a(prm, Ax, (seq - 1u) & 1u, seq - 1u, k, qs, A_s, status);
+          for (int i = tid; i < Ns; i += kThreads) praw_s[i] = (i < ns) ? (double)pk_w[n0 + i] : 0.0;   // (its copy for W is in pt_s)
+          __syncthreads();
+          reg_slice_correct(praw_s, Pc, KV, A_s, ns, k);
+          __syncthreads();
+          if (w == 0) {
+            double q2 = 0.0;
+            for (int u = lane; 2 * u < Ns; u += 32) {
+              const float v0 = (2 * u < ns) ? (float)praw_s[2 * u] : 0.f;
+              const float v1 = (2 * u + 1 < ns) ? (float)praw_s[2 * u + 1] : 0.f;
+              gl_st2(Pfx + (size_t)fpar * ldr + n0 + 2 * u, ll_wordf(v0, ftag), ll_wordf(v1, ftag));
+              q2 += (double)v0 * (double)v0 + (double)v1 * (double)v1;
+            }
+            q2 = warp_sum(q2);
+            if (lane == 0) gl_st2d(Nfx + (size_t)fpar * (Gs * 2) + (size_t)b * 2, q2, ftag);
+          }
+        }
+        if (tid == (kWarps - 1) * 32) {                                       // arrival hint, as in hop 3
+          u64 x = 0, y = 0;
+          gl_wait2(Nfx + (size_t)fpar * (Gs * 2) + (size_t)(Gs - 1) * 2, ftag, x, y, status);
+        }
+        __syncthreads();
+        if (w == kWarps - 1) {
+          double nsum = 0.0;
+          for (int o = lane; o < Gs; o += 32) {
+            u64 x0 = 0, y0 = 0;
+            gl_wait2(Nfx + (size_t)fpar * (Gs * 2) + (size_t)o * 2, ftag, x0, y0, status);
+            nsum += ll_d(x0, y0);
+          }
+          nsum = warp_sum(nsum);
+          if (lane == 0) reinterpret_cast<float*>(ctl_s + 2)[0] = (nsum > 0.0) ? (float)rsqrt(nsum) : 0.f;
+        }
+        {
+          const u64* px = Pfx + (size_t)fpar * ldr;
+          for (int u0 = tid; 2 * u0 < ldr; u0 += kThreads * 4) {
+            u64 x[4], y[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int u = u0 + i * kThreads;
+              x[i] = 0; y[i] = 0;
+              if (2 * u < ldr) gl_ld2(px + 2 * u, x[i], y[i]);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int u = u0 + i * kThreads;
+              if (2 * u < ldr) {
+                gl_wait2(px + 2 * u, ftag, x[i], y[i], status);
+                *reinterpret_cast<float2*>(pk_w + 2 * u) = make_float2(ll_f(x[i]), ll_f(y[i]));
+              }
+            }
+          }
+        }
+        __syncthreads();
+        pscale = reinterpret_cast<const float*>(ctl_s + 2)[0];
+      }
       if (gsk && !owner) {                                                    // everybody needs B for t = t~ - V B
         if (two) {
           const u64* bx = Bx + (size_t)par * (2 + Kpad) * 2;
@@ -750,6 +870,11 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       }
       const float lamf = (float)lam_new;
       const float inv = (float)(1.0 / lam_new);
+      if (gsk) {                                                              // |B_k|^2 of the finished component (every thread: uniform)
+        double bb = 0.0;
+        for (int j = 0; j < k; ++j) bb += B_s[j] * B_s[j];
+        bf2 += bb * (double)rhof * (double)rhof;
+      }
       const float* pk_s = p_s + (size_t)((it - 1) & 1) * ldr;                 // the loads of the last sweep
       // t = t~ - V_(k) B;  GS-PCA: v = t/lambda';  T[:,k] = lambda' v = t (:87,:1037)
       for (int r = w; r < mb; r += kWarps) {
@@ -758,7 +883,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           for (int j = lane; j < k; j += 32) c = fmaf(Vb[(size_t)r * KV + j], (float)B_s[j], c);
         const float corr = (float)warp_sum((double)c);
         if (lane == 0) {
-          const float t = ttil_s[r] - corr;
+          const float t = (ttil_s[r] - corr) * rhof;                          // (products of the last sweep are short by rho)
           d_s[r] = t;                                                         // S9: R -= lambda' v p^T  /  R -= t p^T
           Tb[(size_t)k * M + r] = prm.out_svd ? t * inv : t;                  // SVD output: the unit vector v
           if (gs) Vb[(size_t)r * KV + k] = t * inv;
@@ -770,7 +895,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           if (i < ns) prm.P[(size_t)k * N + n0 + i] = pk;
           if (gs) Pc[(size_t)i * KV + k] = pk;
           if (gs && k + 1 < K)                                                // W_k = R_(k+1)^T v_k
-            Wc[(size_t)i * KV + k] = (float)(pt_s[i] / lam_new - lam_new * (double)pk);
+            Wc[(size_t)i * KV + k] = (float)(pt_s[i] * (double)rhof / lam_new - lam_new * (double)pk);
         }
       }
       if (b == 0 && tid == 0) { prm.lambda[k] = lamf; prm.iters[k] = it; }

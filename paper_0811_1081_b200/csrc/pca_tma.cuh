@@ -66,21 +66,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-// ... with an L2 eviction-priority hint (createpolicy)
-__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, unsigned bytes, void* bar, unsigned long long pol) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
-}
-__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
-  unsigned long long p;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
-  unsigned long long p;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 __device__ __forceinline__ void st_release_cta(unsigned* p, unsigned v) {
   asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
@@ -137,11 +122,6 @@ struct Ring {
   int iss_slot;             // leader: slot of the next batch to issue
   int inflight;             // leader: issued and not yet consumed
   int iss_sw, iss_bq;       // leader: stream position of the next batch to issue
-  // L2 residency control: the last `tail_from..nb` batch positions of a sweep are the head of the next one (opposite row
-  // order); they are fetched with evict_last, everything else with evict_first, so that the 126 MB L2 keeps exactly the
-  // rows that are read again soonest instead of an LRU mix of the stream.  tail_from >= nb: no hints.
-  int tail_from;
-  unsigned long long pol_keep, pol_stream;
 
   __device__ __forceinline__ const float* cur_slot() const { return slots + (size_t)cons_slot * (RB * ldr); }
   __device__ __forceinline__ void wait_next() const { mbar_wait(full + cons_slot, cons_par, status); }   // batch has landed
@@ -158,9 +138,7 @@ struct Ring {
       const unsigned bytes = (unsigned)rows * (unsigned)ldr * 4u;
       unsigned long long* bar = full + iss_slot;
       mbar_expect_tx(bar, bytes);
-      if (tail_from >= nb) bulk_g2s(slots + (size_t)iss_slot * (RB * ldr), Rb + (size_t)r0 * ldr, bytes, bar);
-      else bulk_g2s_hint(slots + (size_t)iss_slot * (RB * ldr), Rb + (size_t)r0 * ldr, bytes, bar,
-                         iss_bq >= tail_from ? pol_keep : pol_stream);
+      bulk_g2s(slots + (size_t)iss_slot * (RB * ldr), Rb + (size_t)r0 * ldr, bytes, bar);
       ++inflight;
       if (++iss_slot == SG) iss_slot = 0;
       iss_bq += NG;
@@ -448,11 +426,11 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
   float* qs = reinterpret_cast<float*>(smem + prm.off_qs);        // NG x ldr group partials
   float* red_s = reinterpret_cast<float*>(smem + prm.off_red);    // 2 x kWarps x RB
   double* sgrp = reinterpret_cast<double*>(smem + prm.off_sgrp);  // NG
-  double* sb_s = reinterpret_cast<double*>(smem + prm.off_B);     // 2 + Kpad: |t~|^2, -, B
-  double* B_s = sb_s + 2;
+  double* sb_s = reinterpret_cast<double*>(smem + prm.off_B);     // 4 + Kpad: |t~|^2, -, |A|^2, -, B
+  double* B_s = sb_s + 4;
   double* A_s = reinterpret_cast<double*>(smem + prm.off_A);      // Kpad
   double* scr = reinterpret_cast<double*>(smem + prm.off_scr);    // kThreads
-  double* ctl_s = scr + kThreads - 4;                             // lambda', decision, 1/|p^| of the current pass
+  double* ctl_s = scr + kThreads - 8;                             // lambda', decision, 1/|p^| of the current pass
   double* praw_s = reinterpret_cast<double*>(smem + prm.off_praw);// Ns: p~ / p^ slice of this owner
   float* lam_s = reinterpret_cast<float*>(smem + prm.off_lam);    // Kpad
   float* ring_s = reinterpret_cast<float*>(smem + prm.off_ring);  // NG x SG slots of RB x ldr floats
@@ -485,18 +463,21 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
   asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
 
   const int npx = Gs * Ns;                                 // exchanged length of p (>= N)
-  const int SBw = 2 + Kpad;
+  const int SBw = 4 + Kpad;
   const bool gs = prm.algo == 1;
   const int n0 = b * Ns;
   const int ns = max(0, min(Ns, N - n0));
   const bool owner = ns > 0;
   unsigned seq = 0;                                        // sweep number; parity selects the exchange buffers
-  unsigned e1 = 0, e2 = 0, e3 = 0;                         // expected values of the three arrival counters
+  unsigned e1 = 0, e2 = 0, e3 = 0, e4 = 0;                 // expected values of the arrival counters
   unsigned* const cnt1 = prm.cnt;
   unsigned* const cnt2 = prm.cnt + 64;
   unsigned* const cnt3 = prm.cnt + 128;
+  unsigned* const cnt4 = prm.cnt + 192;
+  double* praw2_s = praw_s + Ns;                           // second slice buffer (final p^ of a component)
   unsigned* status = prm.status;
   int tn = 0;                                              // trace records written (thread 0 of CTA 0)
+  double bf2 = 0.0;                                        // sum over the finished components of |B_j|^2 (see kDeferKappa)
 
   float* Rb = prm.Rrm + (size_t)m0 * ldr;
   float* Tb = prm.T + m0;
@@ -511,9 +492,6 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
     rg.full = mbar_s + g * SG;
     rg.Rb = Rb; rg.SG = SG; rg.ldr = ldr; rg.mb = mb; rg.nb = (mb + RB - 1) / RB; rg.g = g; rg.NG = NG;
     rg.cons = 0; rg.cons_slot = 0; rg.cons_par = 0u; rg.iss_slot = 0; rg.inflight = 0; rg.iss_sw = 0; rg.iss_bq = g; rg.status = status;
-    rg.tail_from = prm.l2_tail > 0 ? rg.nb - (int)(((long long)rg.nb * prm.l2_tail) / 1000) : rg.nb;
-    rg.pol_keep = l2_policy_evict_last();
-    rg.pol_stream = l2_policy_evict_first();
     if (tid - g * GT == 0) rg.top_up(0);                   // the head of the first sweep is on its way
   }
   int sw = 0;                                              // sweeps done (loads sweeps included): row order of the next one
@@ -556,6 +534,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
     int it = 0;
     bool degenerate = false;
     bool first = true;
+    float inv_pn = 0.f;                                      // 1/|p~| (1/|p^|) of the pass in flight
+    bool deferred = false;                                   // the loads of the pass in flight are p~ (S3 deferred), not p^
     for (;;) {
       const unsigned par = seq & 1u;
       // ---- hop 1: |t~|^2 and B (every CTA), raw loads slice (owners) ----
@@ -565,15 +545,15 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
         LLJob jq, jsb;
         jq.base = prm.Qx + ((size_t)par * Gs + b) * G * Ns; jq.out = praw_s; jq.units = owner ? (Ns >> 1) : 0;
         jq.nparts = G; jq.stride = Ns; jq.f64_unit0 = false;
-        jsb.base = prm.SBx + (size_t)par * G * SBw; jsb.out = sb_s; jsb.units = 1 + ((gsk && !first) ? ((k + 1) >> 1) : 0);
-        jsb.nparts = G; jsb.stride = SBw; jsb.f64_unit0 = true;
+        jsb.base = prm.SBx + (size_t)par * G * SBw; jsb.out = sb_s; jsb.units = (gsk && !first) ? 2 + ((k + 1) >> 1) : 1;
+        jsb.nparts = G; jsb.stride = SBw; jsb.f64_unit0 = 2;
         if (jsb.units <= 16) {
           ll_reduce2(jsb, jq, seq, status);
         } else {
           RegGather gsb;
           int hs = 32;
           while (hs < jsb.units) hs <<= 1;
-          gsb.base = jsb.base; gsb.stride = SBw; gsb.hp = hs; gsb.npairs = jsb.units; gsb.nparts = G; gsb.f64_pair0 = true;
+          gsb.base = jsb.base; gsb.stride = SBw; gsb.hp = hs; gsb.npairs = jsb.units; gsb.nparts = G; gsb.f64_pair0 = 2;
           gsb.red = reinterpret_cast<double2*>(qs); gsb.out = sb_s;
           u64 sx[8], sy[8];
           reg_gather_issue<8>(gsb, sx, sy);
@@ -599,7 +579,23 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
             for (int j = lane; j < k; j += 32) bb += B_s[j] * B_s[j];
             bb = warp_sum(bb);
           }
-          const double l2 = s - bb;                                           // |t~ - V B|^2, V orthonormal
+          double l2 = s - bb;                                                 // |t~ - V B|^2, V orthonormal
+          double rho = 1.0;
+          if (gsk) {
+            const double pn2 = ctl_s[3], a2 = sb_s[2];
+            if (deferred) {
+              // deferred loads-side Gram-Schmidt (see "S3" below): the sweep ran with p~/|p~| instead of p^/|p^|,
+              // |p^|^2 = |p~|^2 - |A|^2 (P orthonormal), so every product of the sweep is short of the paper's by
+              // rho = |p~|/|p^|
+              const double d2 = pn2 - a2;
+              if (!(d2 > 0.0)) l2 = 0.0;
+              else rho = sqrt(pn2 / d2);
+              l2 *= rho * rho;
+            }
+            // the NEXT pass defers S3 only if that is harmless (same decision on every CTA): see kDeferKappa
+            if (lane == 0) reinterpret_cast<int*>(ctl_s + 4)[0] = (a2 * bf2 <= kDeferKappa * pn2 * lam * lam) ? 1 : 0;
+          }
+          if (lane == 0) ctl_s[2] = rho;
           if (!(l2 > 0.0)) st = 2;                                            // reading C7
           else {
             ln = sqrt(l2);                                                    // S7
@@ -639,16 +635,27 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
       if (done) break;
       trace_mark(prm, tn, TR_QSLICE);
 
-      if (gsk && owner) {
-        if (tid == 0) hop_arrive(cnt2);                                       // A-partials of this pass are out
-        trace_mark(prm, tn, TR_APART);
-        e2 += (unsigned)Gs;
+      // ---- S3, deferred.  The paper orthogonalises the loads first, p^ = p~ - P_(k) A, and multiplies
+      // then, t~ = R p^.  R P_(k) lies in span V_(k) (deflation: R_(j+1) p_j = t~_j - t_j = V_(j) B_j, and later deflations
+      // add multiples of v_i), and the scores-side projection t = t~ - V_(k) V_(k)^T t~ removes that
+      // span, so R p~ and R p^ give the SAME t: the sweep can start from p~ without waiting for A = sum of the owners'
+      // partials (one dependent cross-CTA hop less per pass).  What the iteration needs from A is |p^|^2 = |p~|^2 - |A|^2
+      // (lambda' scales with 1/|p^|); it travels with the NEXT exchange.  p^ itself is formed once, when the component has
+      // converged ("final loads" below).  (The two-sweep kernel keeps the paper's literal order.)
+      // Deferring costs accuracy when A is NOT small (the first pass of a component starts from a raw column; fixed-pass
+      // runs never converge): t~ then carries a large component in span V_(k) and lambda'^2 = |t~|^2 - |B|^2 cancels.  So the
+      // first two passes of a component, and every pass for which the bound of kDeferKappa fails, take the paper's order.
+      const bool defer_now = gsk && !first && reinterpret_cast<const int*>(ctl_s + 4)[0] != 0;
+      if (gsk && owner && tid == 0) hop_arrive(cnt2);                         // A-partials of this pass are out
+      trace_mark(prm, tn, TR_APART);
+      if (gsk) e2 += (unsigned)Gs;
+      if (gsk && owner && !defer_now) {
         hop_wait_c(cnt2, e2, status);
         // ---- hop 2: A = sum of the owners' partials;  p^ = p~ - P_(k) A ----
         if (k <= 30) {
           LLJob ja, jn;
           ja.base = prm.Ax + (size_t)par * Gs * Kpad; ja.out = A_s; ja.units = (k + 1) >> 1; ja.nparts = Gs; ja.stride = Kpad;
-          ja.f64_unit0 = false;
+          ja.f64_unit0 = 0;
           jn = ja; jn.units = 0;
           ll_reduce2(ja, jn, seq, status);
         } else {
@@ -657,7 +664,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
           int ha = 32;
           while (ha < ua) ha <<= 1;
           ga.base = prm.Ax + (size_t)par * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
-          ga.f64_pair0 = false; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
+          ga.f64_pair0 = 0; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
           u64 ax8[8], ay8[8];
           reg_gather_issue<8>(ga, ax8, ay8);
           reg_gather_finish<8>(ga, ax8, ay8, seq, status);
@@ -669,7 +676,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
         slice_correct(praw_s, Pc, A_s, ns, k, Kpad);
         cta_sync();
       }
-      // ---- publish the p^ slice and its squared norm (S4, first half) ----
+      deferred = defer_now;
+      // ---- publish the p~ slice and its squared norm (S4, first half) ----
       if (owner && w == 0) {
         double q2 = 0.0;
         for (int u = lane; 2 * u < Ns; u += 32) {
@@ -693,7 +701,27 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
         jn.base = prm.Nx + (size_t)par * Gs * 2; jn.out = scr; jn.units = 1; jn.nparts = Gs; jn.stride = 2; jn.f64_unit0 = true;
         ll_reduce_unit(jn, 0, seq, status);
         __syncwarp();
-        if (lane == 0) reinterpret_cast<float*>(ctl_s + 2)[0] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+        if (lane == 0) {
+          ctl_s[3] = scr[0];                                                  // |p~|^2
+          reinterpret_cast<float*>(ctl_s + 1)[1] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+        }
+      }
+      if (gsk && w == kWarps - 2) {
+        // this CTA's share of |A|^2: the entries A[2u], A[2u+1] of its units u = b, b + G, ... summed over the owners'
+        // partials (fixed order); published with |t~|^2 after the sweep, summed over the CTAs at the next hop 1
+        double a2 = 0.0;
+        LLJob ja;
+        ja.base = prm.Ax + (size_t)par * Gs * Kpad; ja.out = scr + 8; ja.nparts = Gs; ja.stride = Kpad; ja.f64_unit0 = 0;
+        ja.units = (k + 1) >> 1;
+        double* ao = scr + 8;                                                  // (scr[0..] belongs to the norm warp)
+        for (int u = b; u < ja.units; u += G) {
+          ja.out = ao - 2 * u;                                                // the unit's two sums land in ao[0], ao[1]
+          ll_reduce_unit(ja, u, seq, status);
+          __syncwarp();
+          a2 += ao[0] * ao[0] + ao[1] * ao[1];
+          __syncwarp();
+        }
+        if (lane == 0) scr[4] = a2;
       }
       {
         const u64* px = prm.Px + (size_t)par * npx;
@@ -717,7 +745,8 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
       }
       cta_sync();
       trace_mark(prm, tn, TR_X3);
-      const float inv_pn = reinterpret_cast<const float*>(ctl_s + 2)[0];      // p = p^/|p^|
+      inv_pn = reinterpret_cast<const float*>(ctl_s + 1)[1];                  // p = p~/|p~| (see S3 above)
+      const double a2mine = gsk ? scr[4] : 0.0;
       if (!(inv_pn > 0.f)) { degenerate = true; break; }                      // reading C7
       for (int n = tid; n < npx; n += kThreads) p_s[n] *= inv_pn;             // each thread rescales what it wrote
       if (gsk && tid == 0) { cmd_s[0] = HCMD_SWEEP; cmd_s[1] = k; cmd_s[2] = sw; }
@@ -746,6 +775,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
           double a = 0.0;
           for (int g = 0; g < NG; ++g) a += sgrp[g];
           ll_st2d(sbx, a, seq);
+          if (gsk) ll_st2d(sbx + 2, a2mine, seq);
         }
         if (gsk) {
           named_bar_sync(BAR_HDONE, kTmaThreads);                             // the helpers' partial sums are in hb_s
@@ -756,7 +786,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
               s0 += hb_s[(size_t)h * Kpad + j0];
               if (j0 + 1 < k) s1 += hb_s[(size_t)h * Kpad + j0 + 1];
             }
-            ll_st2(sbx + 2 + j0, ll_wordf(s0, seq), ll_wordf(s1, seq));
+            ll_st2(sbx + 4 + j0, ll_wordf(s0, seq), ll_wordf(s1, seq));
           }
         }
         cta_sync();                                                           // all LL stores of this CTA are issued
@@ -765,6 +795,86 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
       }
     }
 
+    if (!degenerate && gsk && deferred) {
+      // ---- final loads (once per component, if the pass that converged had S3 deferred): p^ = p~ - P_(k) A (S3) of the pass that converged,
+      //      p = p^/|p^| (S4).  p_s holds p~/|p~|, the owners' A-partials of that pass are in Ax. ----
+      const unsigned apar = (seq - 1u) & 1u, aseq = seq - 1u;
+      const unsigned fpar = (unsigned)k & 1u, ftag = (unsigned)k + 1u;
+      if (owner) {
+        if (k <= 30) {
+          LLJob ja, jn;
+          ja.base = prm.Ax + (size_t)apar * Gs * Kpad; ja.out = A_s; ja.units = (k + 1) >> 1; ja.nparts = Gs; ja.stride = Kpad;
+          ja.f64_unit0 = 0;
+          jn = ja; jn.units = 0;
+          ll_reduce2(ja, jn, aseq, status);
+        } else {
+          RegGather ga;
+          const int ua = (k + 1) >> 1;
+          int ha = 32;
+          while (ha < ua) ha <<= 1;
+          ga.base = prm.Ax + (size_t)apar * Gs * Kpad; ga.stride = Kpad; ga.hp = ha; ga.npairs = ua; ga.nparts = Gs;
+          ga.f64_pair0 = 0; ga.red = reinterpret_cast<double2*>(qs); ga.out = A_s;
+          u64 ax8[8], ay8[8];
+          reg_gather_issue<8>(ga, ax8, ay8);
+          reg_gather_finish<8>(ga, ax8, ay8, aseq, status);
+          cta_sync();
+          reg_gather_store(ga);
+        }
+        cta_sync();
+        for (int i = tid; i < Ns; i += kThreads) praw2_s[i] = (i < ns) ? (double)p_s[n0 + i] : 0.0;
+        for (int j = tid; j < k; j += kThreads) A_s[j] *= (double)inv_pn;   // A of the scaled vector p~/|p~|
+        cta_sync();
+        slice_correct(praw2_s, Pc, A_s, ns, k, Kpad);
+        cta_sync();
+        if (w == 0) {
+          double q2 = 0.0;
+          for (int u = lane; 2 * u < Ns; u += 32) {
+            const float v0 = (2 * u < ns) ? (float)praw2_s[2 * u] : 0.f;
+            const float v1 = (2 * u + 1 < ns) ? (float)praw2_s[2 * u + 1] : 0.f;
+            ll_st2(prm.Pfx + (size_t)fpar * npx + n0 + 2 * u, ll_wordf(v0, ftag), ll_wordf(v1, ftag));
+            q2 += (double)v0 * (double)v0 + (double)v1 * (double)v1;
+          }
+          q2 = warp_sum(q2);
+          if (lane == 0) {
+            ll_st2d(prm.Nfx + ((size_t)fpar * Gs + b) * 2, q2, ftag);
+            hop_arrive(cnt4);
+          }
+        }
+      }
+      e4 += (unsigned)Gs;
+      hop_wait_c(cnt4, e4, status);
+      if (w == kWarps - 1) {
+        LLJob jn;
+        jn.base = prm.Nfx + (size_t)fpar * Gs * 2; jn.out = scr; jn.units = 1; jn.nparts = Gs; jn.stride = 2; jn.f64_unit0 = 1;
+        ll_reduce_unit(jn, 0, ftag, status);
+        __syncwarp();
+        if (lane == 0) reinterpret_cast<float*>(ctl_s + 1)[1] = (scr[0] > 0.0) ? (float)rsqrt(scr[0]) : 0.f;
+      }
+      {
+        const u64* px = prm.Pfx + (size_t)fpar * npx;
+        for (int u0 = tid; 2 * u0 < npx; u0 += kThreads * 4) {
+          u64 x[4], y[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int u = u0 + i * kThreads;
+            x[i] = 0; y[i] = 0;
+            if (2 * u < npx) ll_ld2(px + 2 * u, x[i], y[i]);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int u = u0 + i * kThreads;
+            if (2 * u < npx) {
+              ll_wait2(px + 2 * u, ftag, x[i], y[i], status);
+              *reinterpret_cast<float2*>(p_s + 2 * u) = make_float2(ll_f(x[i]), ll_f(y[i]));
+            }
+          }
+        }
+      }
+      cta_sync();
+      const float inv_f = reinterpret_cast<const float*>(ctl_s + 1)[1];
+      for (int n = tid; n < npx; n += kThreads) p_s[n] *= inv_f;
+      cta_sync();
+    }
     // ---- component done ----
     if (degenerate) {
       for (int i = tid; i < mb; i += kThreads) {
@@ -779,13 +889,20 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
     } else {
       const float lamf = (float)lam_new;
       const float inv = (float)(1.0 / lam_new);
+      const double rho = (gsk && deferred) ? ctl_s[2] : 1.0;                               // products of the last sweep are short by rho (S3)
+      const float rhof = (float)rho;
+      if (gsk) {                                                              // |B_k|^2 of the finished component (every thread: uniform)
+        double bb = 0.0;
+        for (int j = 0; j < k; ++j) bb += B_s[j] * B_s[j];
+        bf2 += bb * rho * rho;
+      }
       // t = t~ - V_(k) B;  GS-PCA: v = t/lambda'
       for (int i = tid; i < mb; i += kThreads) {
         float t = ttil_s[i];
         if (gsk) {
           float corr = 0.f;
           for (int j = 0; j < k; ++j) corr = fmaf(Tb[(size_t)j * M + i], (float)B_s[j], corr);
-          t -= corr;
+          t = (t - corr) * rhof;
         }
         d_s[i] = t;                                                           // R -= lambda v p^T  /  R -= t p^T
         Tb[(size_t)k * M + i] = (gs || prm.out_svd) ? t * inv : t;
@@ -796,7 +913,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
         prm.P[(size_t)k * N + n0 + tid] = pk;
         Pc[(size_t)tid * Kpad + k] = pk;
         if (gs && k + 1 < K)                                                  // W_k = R_(k+1)^T v_k
-          Wc[(size_t)tid * Kpad + k] = (float)(praw_s[tid] / lam_new - lam_new * (double)pk);
+          Wc[(size_t)tid * Kpad + k] = (float)(praw_s[tid] * rho / lam_new - lam_new * (double)pk);
       }
       for (int n = tid; n < ldr; n += kThreads) pdef_s[n] = (n < npx) ? p_s[n] : 0.f;
       if (b == 0 && tid == 0) { prm.lambda[k] = lamf; prm.iters[k] = it; }

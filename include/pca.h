@@ -83,7 +83,11 @@ enum {
                            into the two-sweep kernel only: the plan falls back to paths 1/2, forcing paths 3-6 gives
                            PCA_EUNSUPPORTED.  Ignored for NIPALS-PCA */
   PCA_OPT_RING_ROWS = 11, /* path 7: rows of R per ring slot (one bulk copy): 0 = auto, 1, 2 or 4 */
-  PCA_OPT_RING_SLOTS = 12 /* path 7: upper bound on the ring slots per row group (0 = auto: what fits, at most 8) */
+  PCA_OPT_RING_SLOTS = 12, /* path 7: upper bound on the ring slots per row group (0 = auto: what fits, at most 8) */
+  PCA_OPT_STORAGE = 14    /* 0 (default): fp32 storage (pca_center / pca_run / pca_residual); 1: fp64 storage and fp64 arithmetic
+                            throughout, the paper's native precision: pca_center_f64 / pca_run_f64 /
+                            pca_residual_f64, run by the two-sweep kernel (the paper's pass shape) instantiated on double
+                            (PCA_INFO_PATH = 8); the fp32 entry points return PCA_EINVAL on such a context and vice versa */
 };
 
 /* Phase ids of the trace records (pca_trace).  One inner pass of the single-sweep kernel is
@@ -108,7 +112,8 @@ enum {
 /* Fields for pca_get_info. */
 enum {
   PCA_INFO_PATH = 1,        /* 1, 2 = two-sweep kernel streaming / resident; 3, 4 = single-sweep kernel streaming / resident;
-                               5 = register-resident single-sweep kernel; 6 = one-CTA single-sweep kernel */
+                               5 = register-resident single-sweep kernel; 6 = one-CTA single-sweep kernel; 7 = single-sweep kernel,
+                               TMA ring; 8 = two-sweep kernel on fp64 storage */
   PCA_INFO_CTAS = 2,        /* CTAs of the persistent solve kernel */
   PCA_INFO_THREADS = 3,     /* threads per CTA */
   PCA_INFO_SMEM_BYTES = 4,  /* dynamic shared memory per CTA */
@@ -185,6 +190,14 @@ int pca_run(pca_ctx*, const float* X, float* T, float* P, float* lambda, int32_t
 /* Pointer to the residual R (dev, M x N, ld = M) inside the workspace; valid after a pca_run on
  * this context has completed ("return T, P, R"). */
 int pca_residual(const pca_ctx*, const float** R);
+
+/* fp64 storage variant (PCA_OPT_STORAGE = 1; the paper works in double precision throughout; SURVEY.md
+ * section 8(f) F3).  Same semantics, layouts, ownership and error behaviour as pca_center / pca_run / pca_residual with every
+ * matrix and vector in double (X, T, P, lambda: dev, column-major, 16-byte aligned); all arithmetic is fp64.  The workspace is
+ * sized for double (pca_workspace_bytes after the option is set).  PCA_EINVAL on a context whose storage option is 0. */
+int pca_center_f64(pca_ctx*, double* X, void* stream);
+int pca_run_f64(pca_ctx*, const double* X, double* T, double* P, double* lambda, int32_t* iters, void* stream);
+int pca_residual_f64(const pca_ctx*, const double** R);
 
 /* Device-side phase trace of the last pca_run (tracing aid; PCA_OPT_TRACE > 0, single-sweep kernels, paths 3-5).
  *   records   dev pointer inside the workspace: records[0] = number of records written per slot,

@@ -20,6 +20,8 @@ PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED, PCA
 
 PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT, PCA_OPT_TEST_MODE = 1, 2, 3, 4, 5, 6, 7
 PCA_OPT_STAGNATION, PCA_OPT_OUTPUT, PCA_OPT_GS_PASSES, PCA_OPT_RING_ROWS, PCA_OPT_RING_SLOTS = 8, 9, 10, 11, 12
+PCA_OPT_STORAGE = 14
+PCA_PATH_F64 = 8
 (PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT,
  PCA_PATH_REGISTER, PCA_PATH_ONE_CTA, PCA_PATH_TMA_STREAMING) = 0, 1, 2, 3, 4, 5, 6, 7
 (PCA_INFO_PATH, PCA_INFO_CTAS, PCA_INFO_THREADS, PCA_INFO_SMEM_BYTES, PCA_INFO_ROWS_PER_CTA,
@@ -29,7 +31,7 @@ PCA_OPT_STAGNATION, PCA_OPT_OUTPUT, PCA_OPT_GS_PASSES, PCA_OPT_RING_ROWS, PCA_OP
 EXPORTED_SYMBOLS = (
     "pca_create", "pca_set_option", "pca_get_info", "pca_workspace_bytes", "pca_set_workspace",
     "pca_center", "pca_run", "pca_residual", "pca_fit_host", "pca_destroy", "pca_strerror",
-    "pca_last_cuda_error", "pca_trace",
+    "pca_last_cuda_error", "pca_trace", "pca_center_f64", "pca_run_f64", "pca_residual_f64",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -71,6 +73,9 @@ def load_library() -> ctypes.CDLL:
     lib.pca_strerror.restype = ctypes.c_char_p
     lib.pca_last_cuda_error.argtypes = [vp]
     lib.pca_trace.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(i64)]
+    lib.pca_center_f64.argtypes = [vp, vp, vp]
+    lib.pca_run_f64.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.pca_residual_f64.argtypes = [vp, ctypes.POINTER(vp)]
     _lib = lib
     return lib
 
@@ -121,7 +126,7 @@ class PcaContext:
             "path": {1: "two-sweep streaming", 2: "two-sweep resident", 3: "single-sweep streaming",
                      4: "single-sweep resident",
                      5: "single-sweep register-resident", 6: "single-sweep one-CTA",
-                     7: "single-sweep streaming (TMA ring)"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
+                     7: "single-sweep streaming (TMA ring)", 8: "two-sweep streaming fp64"}.get(self.pca_get_info(PCA_INFO_PATH), "?"),
             "ctas": self.pca_get_info(PCA_INFO_CTAS),
             "threads": self.pca_get_info(PCA_INFO_THREADS),
             "smem_bytes": self.pca_get_info(PCA_INFO_SMEM_BYTES),
@@ -175,6 +180,32 @@ class PcaContext:
                                  vp(lam.data_ptr()), vp(iters.data_ptr()), _stream_ptr(stream)),
                "pca_run", self._ctx)
 
+    # -- fp64 storage (PCA_OPT_STORAGE = 1): same calls on float64 tensors ----------------------
+    def pca_center_f64(self, X, stream=None) -> None:
+        self._check_mat(X, self.N, self.M, "X", f64=True)
+        _check(self._lib.pca_center_f64(self._ctx, ctypes.c_void_p(X.data_ptr()), _stream_ptr(stream)), "pca_center_f64", self._ctx)
+
+    def pca_run_f64(self, X, T, P, lam, iters, stream=None) -> None:
+        import torch
+        self._check_mat(X, self.N, self.M, "X", f64=True)
+        self._check_mat(T, self.K, self.M, "T", f64=True)
+        self._check_mat(P, self.K, self.N, "P", f64=True)
+        if lam.dtype != torch.float64 or lam.numel() != self.K or not lam.is_cuda or not lam.is_contiguous():
+            raise ValueError("lambda must be a contiguous CUDA float64 tensor of K elements")
+        if iters.dtype != torch.int32 or iters.numel() != self.K or not iters.is_cuda or not iters.is_contiguous():
+            raise ValueError("iters must be a contiguous CUDA int32 tensor of K elements")
+        self.ensure_workspace(X.device)
+        vp = ctypes.c_void_p
+        _check(self._lib.pca_run_f64(self._ctx, vp(X.data_ptr()), vp(T.data_ptr()), vp(P.data_ptr()),
+                                     vp(lam.data_ptr()), vp(iters.data_ptr()), _stream_ptr(stream)), "pca_run_f64", self._ctx)
+
+    def pca_residual_f64(self):
+        import torch
+        ptr = ctypes.c_void_p()
+        _check(self._lib.pca_residual_f64(self._ctx, ctypes.byref(ptr)), "pca_residual_f64")
+        off = ptr.value - self._ws.data_ptr()
+        return self._ws[off:off + self.M * self.N * 8].view(torch.float64).view(self.N, self.M)
+
     def pca_residual(self):
         """View of the residual R inside the workspace as a (N, M) torch tensor (valid after pca_run)."""
         import torch
@@ -209,10 +240,11 @@ class PcaContext:
 
     # -- misc ---------------------------------------------------------------------------------
     @staticmethod
-    def _check_mat(t, rows, cols, name):
+    def _check_mat(t, rows, cols, name, f64=False):
         import torch
-        if (not t.is_cuda) or t.dtype != torch.float32 or tuple(t.shape) != (rows, cols) or not t.is_contiguous():
-            raise ValueError(f"{name} must be a contiguous CUDA float32 tensor of shape ({rows}, {cols})")
+        want = torch.float64 if f64 else torch.float32
+        if (not t.is_cuda) or t.dtype != want or tuple(t.shape) != (rows, cols) or not t.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous CUDA {want} tensor of shape ({rows}, {cols})")
 
     def pca_destroy(self) -> None:
         if getattr(self, "_ctx", None) is not None and self._ctx.value:
@@ -270,5 +302,32 @@ def fit(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, path=P
                Xc=to_colmajor(X), info=ctx.info())
     if want_residual:
         out["R"] = to_colmajor(ctx.pca_residual()).copy()
+    ctx.pca_destroy()
+    return out
+
+
+def fit_f64(X_np, K, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, center=True, ctas=0, want_residual=False, options=None):
+    """fp64-storage sibling of fit(): numpy (M, N) float64 in -> dict of float64 numpy results (PCA_OPT_STORAGE = 1)."""
+    import numpy as np
+    import torch
+    M, N = X_np.shape
+    ctx = PcaContext(M, N, K, eps, max_iter, algo)
+    ctx.pca_set_option(PCA_OPT_STORAGE, 1)
+    if ctas:
+        ctx.pca_set_option(PCA_OPT_CTAS, ctas)
+    for opt, val in (options or {}).items():
+        ctx.pca_set_option(opt, val)
+    X = torch.from_numpy(np.ascontiguousarray(np.asarray(X_np, dtype=np.float64).T)).cuda()
+    if center:
+        ctx.pca_center_f64(X)
+    T = torch.empty((K, M), dtype=torch.float64, device="cuda")
+    P = torch.empty((K, N), dtype=torch.float64, device="cuda")
+    lam = torch.empty(K, dtype=torch.float64, device="cuda")
+    iters = torch.empty(K, dtype=torch.int32, device="cuda")
+    ctx.pca_run_f64(X, T, P, lam, iters)
+    torch.cuda.synchronize()
+    out = dict(T=to_colmajor(T), P=to_colmajor(P), lam=lam.cpu().numpy(), iters=iters.cpu().numpy(), Xc=to_colmajor(X), info=ctx.info())
+    if want_residual:
+        out["R"] = to_colmajor(ctx.pca_residual_f64()).copy()
     ctx.pca_destroy()
     return out

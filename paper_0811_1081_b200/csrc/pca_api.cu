@@ -94,7 +94,7 @@ struct pca_ctx {
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
-  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0;
+  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0, opt_storage = 0;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -107,6 +107,7 @@ struct pca_ctx {
   size_t ws_off_bx = 0;
   const Variant* variant = nullptr;
   SolveParams prm{};
+  pca::SolveParamsT<double> prm64{};   // PCA_OPT_STORAGE = 1
   const FusedVariant* fvariant = nullptr;
   fused_kernel_t ffn = nullptr;      // the kernel of paths 3, 4, 7
   int ring_rows = 0;
@@ -165,7 +166,7 @@ void choose_mapping(int vec, long long rv, int* tr, int* rc) {
 }
 
 // Fill prm's geometry + shared-memory carve-up for a given (path, G).  Returns dynamic smem bytes.
-size_t carve(pca_ctx* c, int resident, int G, int vec, SolveParams* p, int* tr, int* rc) {
+size_t carve(pca_ctx* c, int resident, int G, int vec, SolveParams* p, int* tr, int* rc, size_t esz = 4) {
   const long long M = c->M, N = c->N;
   p->G = G;
   p->Mb = (int)round_up(ceil_div(M, G), vec);
@@ -178,15 +179,15 @@ size_t carve(pca_ctx* c, int resident, int G, int vec, SolveParams* p, int* tr, 
   const int ch = vec * (*tr) * (*rc);
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 16); return (int)o; };
-  p->off_t = take((size_t)round_up(p->Mb, 4) * 4);
-  p->off_d = take((size_t)round_up(p->Mb, 4) * 4);
-  p->off_p = take((size_t)p->Npad * 4);
-  p->off_slice = take((size_t)p->Ns * 4);
+  p->off_t = take((size_t)round_up(p->Mb, 4) * esz);
+  p->off_d = take((size_t)round_up(p->Mb, 4) * esz);
+  p->off_p = take((size_t)p->Npad * esz);
+  p->off_slice = take((size_t)p->Ns * esz);
   p->off_coef = take((size_t)p->Kpad * 8);
-  p->off_lam = take((size_t)p->Kpad * 4);
+  p->off_lam = take((size_t)p->Kpad * esz);
   p->off_scr = take((size_t)pca::kThreads * 8);
-  p->off_red = take((size_t)pca::kWarps * ch * 4);
-  p->off_slab = take(resident ? (size_t)p->slab_ld * (size_t)N * 4 : 0);
+  p->off_red = take((size_t)pca::kWarps * ch * esz);
+  p->off_slab = take(resident ? (size_t)p->slab_ld * (size_t)N * esz : 0);
   return off;
 }
 
@@ -527,8 +528,56 @@ int make_one_plan(pca_ctx* c) {
   return PCA_OK;
 }
 
+// fp64 storage (PCA_OPT_STORAGE = 1): the two-sweep streaming kernel instantiated on double (path 8)
+int make_f64_plan(pca_ctx* c) {
+  if (c->opt_path != 0 && c->opt_path != 1 && c->opt_path != 8) return PCA_EUNSUPPORTED;
+  const long long M = c->M, N = c->N;
+  const int sms = c->num_sms;
+  const int g_min = (int)ceil_div(N, pca::kThreads);
+  if (g_min > sms) return PCA_EUNSUPPORTED;
+  int G = c->opt_ctas > 0 ? c->opt_ctas : sms;
+  if (G < g_min) G = g_min;
+  if (G > sms) G = sms;
+  SolveParams g{};
+  int tr = 0, rc = 0;
+  const size_t smem = carve(c, 0, G, 1, &g, &tr, &rc, 8);
+  if (smem > (size_t)c->smem_optin || tr != 32 || rc != 4) return PCA_EUNSUPPORTED;
+  cudaError_t e = cudaFuncSetAttribute(pca::pca_solve_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pca::pca_solve_f64_kernel, pca::kThreads, smem);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  if ((long long)per_sm * sms < g.G) return PCA_EUNSUPPORTED;
+  pca::SolveParamsT<double> p{};
+  p.M = M; p.N = N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode;
+  p.stag2 = c->opt_stag2; p.out_svd = c->opt_output; p.gs_passes = c->opt_gs_passes;
+  p.G = g.G; p.Mb = g.Mb; p.Ns = g.Ns; p.Gs = g.Gs; p.slab_ld = 0; p.Npad = g.Npad; p.Kpad = g.Kpad;
+  p.off_t = g.off_t; p.off_d = g.off_d; p.off_p = g.off_p; p.off_slice = g.off_slice; p.off_coef = g.off_coef;
+  p.off_lam = g.off_lam; p.off_scr = g.off_scr; p.off_red = g.off_red; p.off_slab = g.off_slab;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
+  take((size_t)M * (size_t)N * 8);                                   // residual of eq. (4), column-major, double
+  c->ws_off_ppart = take((size_t)p.G * p.Npad * 8);
+  c->ws_off_apart = take((size_t)2 * p.Gs * p.Kpad * 8);
+  c->ws_off_bpart = take((size_t)2 * p.G * p.Kpad * 8);
+  c->ws_off_pvec = take((size_t)p.Npad * 8);
+  c->ws_off_qpart = take((size_t)p.Gs * 8);
+  c->ws_off_spart = take((size_t)p.G * 8);
+  c->ws_off_bar = take(256);
+  c->ws_bytes = off;
+  c->prm64 = p;
+  c->smem_bytes = smem;
+  c->path = 8;
+  c->planned = true;
+  c->ws = nullptr;
+  c->ws_given = 0;
+  c->ran = false;
+  return PCA_OK;
+}
+
 int make_plan(pca_ctx* c) {
   c->planned = false;
+  if (c->opt_storage == 1) return make_f64_plan(c);
   // CGS2 (PCA_OPT_GS_PASSES = 2) is built into the two-sweep kernel only (paths 1, 2), whose pass has a separate phase
   // per projection; the single-sweep kernels fold the scores-side projection into the loads by linearity and have no
   // place for a second one.
@@ -623,7 +672,7 @@ int make_plan(pca_ctx* c) {
 int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
   switch (option) {
     case PCA_OPT_PATH:
-      if (value < 0 || value > 7) return PCA_EINVAL;
+      if (value < 0 || value > 8) return PCA_EINVAL;
       c->opt_path = (int)value;
       break;
     case PCA_OPT_CTAS:
@@ -669,6 +718,10 @@ int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
     case PCA_OPT_RING_SLOTS:
       if (value < 0 || value > 8) return PCA_EINVAL;
       c->opt_ring_slots = (int)value;
+      break;
+    case PCA_OPT_STORAGE:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_storage = (int)value;
       break;
     default:
       return PCA_EINVAL;
@@ -720,6 +773,17 @@ int pca_set_option(pca_ctx* c, int option, int64_t value) {
 
 int pca_get_info(const pca_ctx* c, int field, int64_t* value) {
   if (!c || !value || !c->planned) return PCA_EINVAL;
+  if (c->path == 8) {                                              // fp64 two-sweep kernel
+    switch (field) {
+      case PCA_INFO_PATH: *value = 8; return PCA_OK;
+      case PCA_INFO_CTAS: *value = c->prm64.G; return PCA_OK;
+      case PCA_INFO_OWNERS: *value = c->prm64.Gs; return PCA_OK;
+      case PCA_INFO_ROWS_PER_CTA: *value = c->prm64.Mb; return PCA_OK;
+      case PCA_INFO_LAUNCHES_PER_RUN: *value = 1; return PCA_OK;
+      case PCA_INFO_ROW_GROUP_THREADS: case PCA_INFO_RING_ROWS: case PCA_INFO_RING_SLOTS: case PCA_INFO_RUN_STATUS: *value = 0; return PCA_OK;
+      default: break;
+    }
+  }
   switch (field) {
     case PCA_INFO_PATH: *value = c->path; break;
     case PCA_INFO_CTAS: *value = c->path == 6 ? 1 : c->path == 5 ? c->rprm.G : (c->path >= 3 ? c->fprm.G : c->prm.G); break;
@@ -774,8 +838,58 @@ int pca_center(pca_ctx* c, float* X, void* stream) {
   return PCA_OK;
 }
 
+int pca_center_f64(pca_ctx* c, double* X, void* stream) {
+  if (!c || !X) return PCA_EINVAL;
+  if (!aligned16(X)) return PCA_EALIGN;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (c->opt_center_mode == 0) {
+    const int grid = (int)(c->N < (long long)c->num_sms * 4 ? c->N : (long long)c->num_sms * 4);
+    pca::pca_center_columns_f64_kernel<<<grid, pca::kCenterThreads, 0, st>>>(X, c->M, (int)c->N);
+  } else {
+    const long long grid = (c->M + 255) / 256;
+    pca::pca_center_eq1_f64_kernel<<<(unsigned)grid, 256, 0, st>>>(X, c->M, (int)c->N);
+  }
+  PCA_CUDA(c, cudaGetLastError());
+  return PCA_OK;
+}
+
+int pca_run_f64(pca_ctx* c, const double* X, double* T, double* P, double* lambda, int32_t* iters, void* stream) {
+  if (!c || !X || !T || !P || !lambda || !iters || !c->planned) return PCA_EINVAL;
+  if (c->path != 8) return PCA_EINVAL;                             // needs PCA_OPT_STORAGE = 1
+  if (!aligned16(X) || !aligned16(T) || !aligned16(P)) return PCA_EALIGN;
+  if (!c->ws || c->ws_given < c->ws_bytes) return PCA_EWORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  unsigned char* ws = static_cast<unsigned char*>(c->ws);
+  pca::SolveParamsT<double> p = c->prm64;
+  p.X = X;
+  p.R = reinterpret_cast<double*>(ws);
+  p.Tm = T; p.P = P; p.lambda = lambda; p.iters = iters;
+  p.Ppart = reinterpret_cast<double*>(ws + c->ws_off_ppart);
+  p.Apart = reinterpret_cast<double*>(ws + c->ws_off_apart);
+  p.Bpart = reinterpret_cast<double*>(ws + c->ws_off_bpart);
+  p.pvec = reinterpret_cast<double*>(ws + c->ws_off_pvec);
+  p.qpart = reinterpret_cast<double*>(ws + c->ws_off_qpart);
+  p.spart = reinterpret_cast<double*>(ws + c->ws_off_spart);
+  p.bar = reinterpret_cast<unsigned long long*>(ws + c->ws_off_bar);
+  PCA_CUDA(c, cudaMemsetAsync(p.bar, 0, 256, st));
+  void* args[] = {&p};
+  PCA_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(pca::pca_solve_f64_kernel), dim3((unsigned)p.G),
+                                          dim3(pca::kThreads), args, c->smem_bytes, st));
+  c->ran = true;
+  return PCA_OK;
+}
+
+int pca_residual_f64(const pca_ctx* c, const double** R) {
+  if (!c || !R) return PCA_EINVAL;
+  if (c->path != 8) return PCA_EINVAL;
+  if (!c->ws || !c->ran) return PCA_EWORKSPACE;
+  *R = reinterpret_cast<const double*>(c->ws);
+  return PCA_OK;
+}
+
 int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32_t* iters, void* stream) {
   if (!c || !X || !T || !P || !lambda || !iters || !c->planned) return PCA_EINVAL;
+  if (c->path == 8) return PCA_EINVAL;                             // fp64 storage: pca_run_f64
   if (!aligned16(X) || !aligned16(T) || !aligned16(P)) return PCA_EALIGN;
   if (!c->ws || c->ws_given < c->ws_bytes) return PCA_EWORKSPACE;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
@@ -862,7 +976,7 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
   SolveParams p = c->prm;
   p.X = X;
   p.R = reinterpret_cast<float*>(ws);
-  p.T = T; p.P = P; p.lambda = lambda; p.iters = iters;
+  p.Tm = T; p.P = P; p.lambda = lambda; p.iters = iters;
   p.Ppart = reinterpret_cast<float*>(ws + c->ws_off_ppart);
   p.Apart = reinterpret_cast<double*>(ws + c->ws_off_apart);
   p.Bpart = reinterpret_cast<double*>(ws + c->ws_off_bpart);
@@ -880,6 +994,7 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
 
 int pca_residual(const pca_ctx* c, const float** R) {
   if (!c || !R) return PCA_EINVAL;
+  if (c->path == 8) return PCA_EINVAL;
   if (!c->ws || !c->ran) return PCA_EWORKSPACE;
   *R = reinterpret_cast<const float*>(c->ws);
   return PCA_OK;
@@ -887,7 +1002,7 @@ int pca_residual(const pca_ctx* c, const float** R) {
 
 int pca_trace(const pca_ctx* c, const uint64_t** records, int64_t* capacity) {
   if (!c || !records || !capacity) return PCA_EINVAL;
-  if (!c->planned || c->path < 3 || c->path == 6 || c->opt_trace <= 0) return PCA_EUNSUPPORTED;
+  if (!c->planned || c->path < 3 || c->path == 6 || c->path == 8 || c->opt_trace <= 0) return PCA_EUNSUPPORTED;
   if (!c->ws || !c->ran) return PCA_EWORKSPACE;
   *records = reinterpret_cast<const uint64_t*>(static_cast<const unsigned char*>(c->ws) + c->ws_off_trace);
   *capacity = c->opt_trace;
@@ -897,6 +1012,7 @@ int pca_trace(const pca_ctx* c, const uint64_t** records, int64_t* capacity) {
 int pca_fit_host(pca_ctx* c, const float* X_host, float* T_host, float* P_host, float* lambda_host,
                  int32_t* iters_host, void* stream) {
   if (!c || !X_host || !T_host || !P_host || !lambda_host || !iters_host || !c->planned) return PCA_EINVAL;
+  if (c->path == 8) return PCA_EUNSUPPORTED;                       // host-buffer entry point: fp32 storage only
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const size_t xb = (size_t)c->M * (size_t)c->N * 4, tb = (size_t)c->M * c->K * 4, pb = (size_t)c->N * c->K * 4;
   // staging buffers (shape-dependent only; one pointer at a time so that a failed allocation is retried, not skipped)

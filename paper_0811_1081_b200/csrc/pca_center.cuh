@@ -76,4 +76,41 @@ __global__ void __launch_bounds__(256) pca_center_eq1_kernel(float* __restrict__
   }
 }
 
+// fp64 storage (the paper's precision): same two kernels on double data
+__global__ void __launch_bounds__(kCenterThreads) pca_center_columns_f64_kernel(double* __restrict__ X, long long M, int N) {
+  __shared__ double red[kCenterThreads / 32 + 1];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  for (int n = blockIdx.x; n < N; n += gridDim.x) {
+    double* col = X + (size_t)n * M;
+    double s = 0.0;
+    for (long long i = tid; i < M; i += kCenterThreads) s += __ldcg(col + i);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    __syncthreads();
+    if (lane == 0) red[w] = s;
+    __syncthreads();
+    if (w == 0) {
+      double t = (lane < kCenterThreads / 32) ? red[lane] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+      if (lane == 0) red[kCenterThreads / 32] = t / (double)M;
+    }
+    __syncthreads();
+    const double mu = red[kCenterThreads / 32];
+    for (long long i = tid; i < M; i += kCenterThreads) col[i] = __ldcg(col + i) - mu;
+  }
+}
+
+__global__ void __launch_bounds__(256) pca_center_eq1_f64_kernel(double* __restrict__ X, long long M, int N) {
+  const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= M) return;
+  double u = 0.0;
+  for (int n = 0; n < N; ++n) u += __ldcg(X + (size_t)n * M + m);
+  const double mean = u / (double)N;
+  for (int n = 0; n < N; ++n) {
+    double* p = X + (size_t)n * M + m;
+    *p = __ldcg(p) - mean;
+  }
+}
+
 }  // namespace pca

@@ -34,30 +34,37 @@ __device__ __forceinline__ float4 ld_cg4(const float* p) {
   return __ldcg(reinterpret_cast<const float4*>(p));
 }
 
-template <int VEC>
-__device__ __forceinline__ void load_vec(float (&x)[VEC], const float* p) {
-  if constexpr (VEC == 4) {
-    const float4 v = ld_cg4(p);
+// T = float (fp32 storage, the build's default) or double (the paper's native precision: VEC = 1)
+__device__ __forceinline__ float fma_t(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_t(double a, double b, double c) { return fma(a, b, c); }
+
+template <typename T, int VEC>
+__device__ __forceinline__ void load_vec(T (&x)[VEC], const T* p) {
+  if constexpr (VEC == 4 && sizeof(T) == 4) {
+    const float4 v = ld_cg4(reinterpret_cast<const float*>(p));
     x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
   } else {
-    x[0] = ld_cg(p);
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) x[e] = ld_cg(p + e);
   }
 }
-template <int VEC>
-__device__ __forceinline__ void load_vec_smem(float (&x)[VEC], const float* p) {
-  if constexpr (VEC == 4) {
+template <typename T, int VEC>
+__device__ __forceinline__ void load_vec_smem(T (&x)[VEC], const T* p) {
+  if constexpr (VEC == 4 && sizeof(T) == 4) {
     const float4 v = *reinterpret_cast<const float4*>(p);
     x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
   } else {
-    x[0] = *p;
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) x[e] = p[e];
   }
 }
-template <int VEC>
-__device__ __forceinline__ void store_vec(float* p, const float (&x)[VEC]) {
-  if constexpr (VEC == 4) {
+template <typename T, int VEC>
+__device__ __forceinline__ void store_vec(T* p, const T (&x)[VEC]) {
+  if constexpr (VEC == 4 && sizeof(T) == 4) {
     *reinterpret_cast<float4*>(p) = make_float4(x[0], x[1], x[2], x[3]);
   } else {
-    *p = x[0];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) p[e] = x[e];
   }
 }
 
@@ -166,11 +173,11 @@ __device__ __forceinline__ void reduce_coef_parts(double* out_s, const double* p
 //   mb           rows this CTA owns;  N columns
 //   t_s, d_s     shared: the CTA's rows of t and of the deflation vector;  pdef_s shared: N floats
 //   part_out     global, N floats: this CTA's partial loads (written by lane lr == 0)
-template <int VEC, int TR, int RC, int SRC, int DST, bool DEFL, bool DOT>
-__device__ __forceinline__ void pass_t(const float* __restrict__ gsrc, float* __restrict__ gdst, long long ld,
-                                       float* slab, int slab_ld, int mb, int N,
-                                       const float* t_s, const float* d_s, const float* pdef_s,
-                                       float* __restrict__ part_out) {
+template <typename T, int VEC, int TR, int RC, int SRC, int DST, bool DEFL, bool DOT>
+__device__ __forceinline__ void pass_t(const T* __restrict__ gsrc, T* __restrict__ gdst, long long ld,
+                                       T* slab, int slab_ld, int mb, int N,
+                                       const T* t_s, const T* d_s, const T* pdef_s,
+                                       T* __restrict__ part_out) {
   constexpr int CW = 32 / TR;
   constexpr int CH = VEC * TR * RC;                    // rows per chunk
   constexpr int U = (RC >= 4) ? 2 : (RC == 2 ? 4 : 8);  // column groups in flight per warp
@@ -179,7 +186,7 @@ __device__ __forceinline__ void pass_t(const float* __restrict__ gsrc, float* __
   const int ngroups = (N + CW - 1) / CW;
 
   for (int r0 = 0; r0 < mb; r0 += CH) {
-    float tv[RC][VEC], dv[RC][VEC];
+    T tv[RC][VEC], dv[RC][VEC];
     int roff[RC];
     bool rok[RC];
 #pragma unroll
@@ -188,12 +195,12 @@ __device__ __forceinline__ void pass_t(const float* __restrict__ gsrc, float* __
       rok[j] = roff[j] < mb;
 #pragma unroll
       for (int e = 0; e < VEC; ++e) {
-        tv[j][e] = (DOT && rok[j]) ? t_s[roff[j] + e] : 0.f;
-        dv[j][e] = (DEFL && rok[j]) ? d_s[roff[j] + e] : 0.f;
+        tv[j][e] = (DOT && rok[j]) ? t_s[roff[j] + e] : T(0);
+        dv[j][e] = (DEFL && rok[j]) ? d_s[roff[j] + e] : T(0);
       }
     }
     for (int g0 = w; g0 < ngroups; g0 += kWarps * U) {
-      float x[U][RC][VEC];
+      T x[U][RC][VEC];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int c = (g0 + u * kWarps) * CW + lc;
@@ -201,11 +208,11 @@ __device__ __forceinline__ void pass_t(const float* __restrict__ gsrc, float* __
 #pragma unroll
         for (int j = 0; j < RC; ++j) {
           if (cok && rok[j]) {
-            if constexpr (SRC == SRC_GLOBAL) load_vec<VEC>(x[u][j], gsrc + (size_t)c * ld + roff[j]);
-            else load_vec_smem<VEC>(x[u][j], slab + (size_t)c * slab_ld + roff[j]);
+            if constexpr (SRC == SRC_GLOBAL) load_vec<T, VEC>(x[u][j], gsrc + (size_t)c * ld + roff[j]);
+            else load_vec_smem<T, VEC>(x[u][j], slab + (size_t)c * slab_ld + roff[j]);
           } else {
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) x[u][j][e] = 0.f;
+            for (int e = 0; e < VEC; ++e) x[u][j][e] = T(0);
           }
         }
       }
@@ -213,23 +220,23 @@ __device__ __forceinline__ void pass_t(const float* __restrict__ gsrc, float* __
       for (int u = 0; u < U; ++u) {
         const int c = (g0 + u * kWarps) * CW + lc;
         const bool cok = c < N;
-        float acc = 0.f;
-        const float pc = (DEFL && cok) ? pdef_s[c] : 0.f;
+        T acc = T(0);
+        const T pc = (DEFL && cok) ? pdef_s[c] : T(0);
 #pragma unroll
         for (int j = 0; j < RC; ++j) {
           if constexpr (DEFL) {
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) x[u][j][e] = fmaf(-dv[j][e], pc, x[u][j][e]);
+            for (int e = 0; e < VEC; ++e) x[u][j][e] = fma_t(-dv[j][e], pc, x[u][j][e]);
           }
           if constexpr (DST != DST_NONE) {
             if (cok && rok[j]) {
-              if constexpr (DST == DST_GLOBAL) store_vec<VEC>(gdst + (size_t)c * ld + roff[j], x[u][j]);
-              else store_vec<VEC>(slab + (size_t)c * slab_ld + roff[j], x[u][j]);
+              if constexpr (DST == DST_GLOBAL) store_vec<T, VEC>(gdst + (size_t)c * ld + roff[j], x[u][j]);
+              else store_vec<T, VEC>(slab + (size_t)c * slab_ld + roff[j], x[u][j]);
             }
           }
           if constexpr (DOT) {
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) acc = fmaf(x[u][j][e], tv[j][e], acc);
+            for (int e = 0; e < VEC; ++e) acc = fma_t(x[u][j][e], tv[j][e], acc);
           }
         }
         if constexpr (DOT) {
@@ -250,9 +257,9 @@ __device__ __forceinline__ void pass_t(const float* __restrict__ gsrc, float* __
 // Columns are walked in DESCENDING order so that (streaming path) the columns the preceding
 // ascending pass_t touched last are re-read while still in L2.
 //   red_s  shared, kWarps * CH floats
-template <int VEC, int TR, int RC, int SRC>
-__device__ __forceinline__ void pass_n(const float* __restrict__ gsrc, long long ld, const float* slab, int slab_ld,
-                                       int mb, int N, const float* p_s, float* t_out_s, float* red_s) {
+template <typename T, int VEC, int TR, int RC, int SRC>
+__device__ __forceinline__ void pass_n(const T* __restrict__ gsrc, long long ld, const T* slab, int slab_ld,
+                                       int mb, int N, const T* p_s, T* t_out_s, T* red_s) {
   constexpr int CW = 32 / TR;
   constexpr int CH = VEC * TR * RC;
   constexpr int U = (RC >= 4) ? 2 : (RC == 2 ? 4 : 8);
@@ -264,31 +271,31 @@ __device__ __forceinline__ void pass_n(const float* __restrict__ gsrc, long long
   for (int r0 = 0; r0 < mb; r0 += CH) {
     int roff[RC];
     bool rok[RC];
-    float acc[RC][VEC];
+    T acc[RC][VEC];
 #pragma unroll
     for (int j = 0; j < RC; ++j) {
       roff[j] = r0 + (lr + TR * j) * VEC;
       rok[j] = roff[j] < mb;
 #pragma unroll
-      for (int e = 0; e < VEC; ++e) acc[j][e] = 0.f;
+      for (int e = 0; e < VEC; ++e) acc[j][e] = T(0);
     }
     for (int s = nsteps - 1; s >= 0; --s) {
       const int g0 = w + s * kWarps * U;
-      float x[U][RC][VEC];
-      float pc[U];
+      T x[U][RC][VEC];
+      T pc[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int c = (g0 + (U - 1 - u) * kWarps) * CW + lc;
         const bool cok = c < N;
-        pc[u] = cok ? p_s[c] : 0.f;
+        pc[u] = cok ? p_s[c] : T(0);
 #pragma unroll
         for (int j = 0; j < RC; ++j) {
           if (cok && rok[j]) {
-            if constexpr (SRC == SRC_GLOBAL) load_vec<VEC>(x[u][j], gsrc + (size_t)c * ld + roff[j]);
-            else load_vec_smem<VEC>(x[u][j], slab + (size_t)c * slab_ld + roff[j]);
+            if constexpr (SRC == SRC_GLOBAL) load_vec<T, VEC>(x[u][j], gsrc + (size_t)c * ld + roff[j]);
+            else load_vec_smem<T, VEC>(x[u][j], slab + (size_t)c * slab_ld + roff[j]);
           } else {
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) x[u][j][e] = 0.f;
+            for (int e = 0; e < VEC; ++e) x[u][j][e] = T(0);
           }
         }
       }
@@ -297,7 +304,7 @@ __device__ __forceinline__ void pass_n(const float* __restrict__ gsrc, long long
 #pragma unroll
         for (int j = 0; j < RC; ++j)
 #pragma unroll
-          for (int e = 0; e < VEC; ++e) acc[j][e] = fmaf(x[u][j][e], pc[u], acc[j][e]);
+          for (int e = 0; e < VEC; ++e) acc[j][e] = fma_t(x[u][j][e], pc[u], acc[j][e]);
     }
     // combine the CW column groups of a warp, then the warps
 #pragma unroll
@@ -316,7 +323,7 @@ __device__ __forceinline__ void pass_n(const float* __restrict__ gsrc, long long
     __syncthreads();
     for (int r = threadIdx.x; r < CH; r += kThreads) {
       if (r0 + r < mb) {
-        float s = 0.f;
+        T s = T(0);
 #pragma unroll
         for (int q = 0; q < kWarps; ++q) s += red_s[q * CH + r];
         t_out_s[r0 + r] = s;

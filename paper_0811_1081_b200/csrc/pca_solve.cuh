@@ -25,12 +25,14 @@
 
 namespace pca {
 
-struct SolveParams {
-  const float* X;        // M x N centred input (never written)
-  float* R;              // M x N residual workspace
-  float* T;              // M x K
-  float* P;              // N x K
-  float* lambda;         // K
+// T = float: fp32 storage (BASELINE.json); T = double: the paper's native precision, everything in fp64
+template <typename T>
+struct SolveParamsT {
+  const T* X;        // M x N centred input (never written)
+  T* R;              // M x N residual workspace
+  T* Tm;             // M x K
+  T* P;              // N x K
+  T* lambda;         // K
   int* iters;            // K
   long long M, N;
   int K;
@@ -49,29 +51,30 @@ struct SolveParams {
   int slab_ld;           // resident path: column stride of the SMEM slab (floats)
   int Npad;              // row stride of Ppart (floats)
   int Kpad;              // row stride of Apart / Bpart (doubles)
-  float* Ppart;          // [G][Npad]   partial loads
+  T* Ppart;          // [G][Npad]   partial loads
   double* Apart;         // [2][Gs][Kpad]  partial A (loads-side GS coefficients), one buffer per CGS projection
   double* Bpart;         // [2][G][Kpad]   partial B (scores-side GS coefficients)
-  float* pvec;           // [Npad]      p^ (orthogonalised, not yet normalised)
+  T* pvec;           // [Npad]      p^ (orthogonalised, not yet normalised)
   double* qpart;         // [Gs]        ||p^||^2 partials
   double* spart;         // [G]         ||t||^2 partials
   unsigned long long* bar;  // grid barrier counter (zeroed before launch)
   // shared memory carve-up (bytes from the start of dynamic smem), computed by the host plan
   int off_t, off_d, off_p, off_slice, off_coef, off_lam, off_scr, off_red, off_slab;
 };
+typedef SolveParamsT<float> SolveParams;
 
-template <bool RESIDENT, int VEC, int TR, int RC>
-__global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParams prm) {
+template <typename T, bool RESIDENT, int VEC, int TR, int RC>
+__device__ __forceinline__ void pca_solve_body(const SolveParamsT<T>& prm) {
   extern __shared__ __align__(16) unsigned char smem[];
-  float* t_s = reinterpret_cast<float*>(smem + prm.off_t);          // Mb: this CTA's rows of t / v
-  float* d_s = reinterpret_cast<float*>(smem + prm.off_d);          // Mb: deflation vector rows
-  float* p_s = reinterpret_cast<float*>(smem + prm.off_p);          // N : full loads vector
-  float* slice_s = reinterpret_cast<float*>(smem + prm.off_slice);  // Ns: this CTA's slice of p~ / p^
+  T* t_s = reinterpret_cast<T*>(smem + prm.off_t);          // Mb: this CTA's rows of t / v
+  T* d_s = reinterpret_cast<T*>(smem + prm.off_d);          // Mb: deflation vector rows
+  T* p_s = reinterpret_cast<T*>(smem + prm.off_p);          // N : full loads vector
+  T* slice_s = reinterpret_cast<T*>(smem + prm.off_slice);  // Ns: this CTA's slice of p~ / p^
   double* coef_s = reinterpret_cast<double*>(smem + prm.off_coef);  // K : A or B
-  float* lam_s = reinterpret_cast<float*>(smem + prm.off_lam);      // K : lambda_k (GS final scaling)
+  T* lam_s = reinterpret_cast<T*>(smem + prm.off_lam);      // K : lambda_k (GS final scaling)
   double* scr = reinterpret_cast<double*>(smem + prm.off_scr);      // kThreads doubles scratch
-  float* red_s = reinterpret_cast<float*>(smem + prm.off_red);      // kWarps * CH floats
-  float* slab = reinterpret_cast<float*>(smem + prm.off_slab);      // resident slab [N][slab_ld]
+  T* red_s = reinterpret_cast<T*>(smem + prm.off_red);      // kWarps * CH floats
+  T* slab = reinterpret_cast<T*>(smem + prm.off_slab);      // resident slab [N][slab_ld]
 
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int b = blockIdx.x;
@@ -85,23 +88,23 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
   const int slab_ld = prm.slab_ld;
   unsigned long long bar_target = 0;
 
-  const float* Xb = prm.X + m0;          // row-offset views (column stride M)
-  float* Rb = prm.R + m0;
-  float* Tb = prm.T + m0;
-  float* my_part = prm.Ppart + (size_t)b * prm.Npad;
+  const T* Xb = prm.X + m0;          // row-offset views (column stride M)
+  T* Rb = prm.R + m0;
+  T* Tb = prm.Tm + m0;
+  T* my_part = prm.Ppart + (size_t)b * prm.Npad;
 
-  for (int i = tid; i < prm.Mb; i += kThreads) d_s[i] = 0.f;
-  for (int n = tid; n < N; n += kThreads) p_s[n] = 0.f;
+  for (int i = tid; i < prm.Mb; i += kThreads) d_s[i] = T(0);
+  for (int n = tid; n < N; n += kThreads) p_s[n] = T(0);
   __syncthreads();
 
   for (int k = 0; k < K; ++k) {
     // ---- S1: t <- R^(k) of the deflated residual (reading C6) ----
     for (int i = tid; i < mb; i += kThreads) {
-      float r;
+      T r;
       if (k == 0) r = ld_cg(Xb + i);                                   // R <- X not yet materialised
       else if constexpr (RESIDENT) r = slab[(size_t)k * slab_ld + i];
       else r = ld_cg(Rb + (size_t)k * M + i);
-      t_s[i] = fmaf(-d_s[i], p_s[k], r);                               // pending deflation of comp k-1
+      t_s[i] = fma_t(-d_s[i], p_s[k], r);                               // pending deflation of comp k-1
     }
     __syncthreads();
 
@@ -112,16 +115,16 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       // ---- Ph1: partial loads (S2), fused with deflation / copy on the first pass (S9, A2) ----
       if (j == 0) {
         if constexpr (RESIDENT) {
-          if (k == 0) pass_t<VEC, TR, RC, SRC_GLOBAL, DST_SLAB, true, true>(Xb, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
-          else        pass_t<VEC, TR, RC, SRC_SLAB, DST_SLAB, true, true>(nullptr, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+          if (k == 0) pass_t<T, VEC, TR, RC, SRC_GLOBAL, DST_SLAB, true, true>(Xb, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+          else        pass_t<T, VEC, TR, RC, SRC_SLAB, DST_SLAB, true, true>(nullptr, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
         } else {
-          pass_t<VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, true>(k == 0 ? Xb : Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
+          pass_t<T, VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, true>(k == 0 ? Xb : Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
         }
       } else {
-        if constexpr (RESIDENT) pass_t<VEC, TR, RC, SRC_SLAB, DST_NONE, false, true>(nullptr, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
-        else                    pass_t<VEC, TR, RC, SRC_GLOBAL, DST_NONE, false, true>(Rb, nullptr, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
+        if constexpr (RESIDENT) pass_t<T, VEC, TR, RC, SRC_SLAB, DST_NONE, false, true>(nullptr, nullptr, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+        else                    pass_t<T, VEC, TR, RC, SRC_GLOBAL, DST_NONE, false, true>(Rb, nullptr, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
       }
-      if (mb == 0) for (int n = tid; n < N; n += kThreads) my_part[n] = 0.f;   // CTA without rows
+      if (mb == 0) for (int n = tid; n < N; n += kThreads) my_part[n] = T(0);   // CTA without rows
       grid_barrier(prm.bar, bar_target, G);
 
       // ---- Ph2: slice owners reduce the G partials: p~[n] = sum_b pp_b[n] ----
@@ -136,7 +139,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
         if (tid < ns) {
           double s = 0.0;
           for (int q = 0; q < nsub; ++q) s += scr[q * ns + tid];
-          slice_s[tid] = (float)s;
+          slice_s[tid] = (T)s;
         }
         __syncthreads();
       }
@@ -146,7 +149,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
           // ---- S3: A-partials  a_b[jj] = sum_{n in slice} P[n,jj] p~[n] ----
           if (ns > 0) {
             for (int jj = tid; jj < k; jj += kThreads) {
-              const float* pj = prm.P + (size_t)jj * N + n0;
+              const T* pj = prm.P + (size_t)jj * N + n0;
               double a = 0.0;
               for (int i = 0; i < ns; ++i) a += (double)ld_cg(pj + i) * (double)slice_s[i];
               Apart[(size_t)b * prm.Kpad + jj] = a;
@@ -167,7 +170,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
             if (tid < ns) {
               double s = 0.0;
               for (int q = 0; q < nsub; ++q) s += scr[q * ns + tid];
-              slice_s[tid] = (float)((double)slice_s[tid] - s);
+              slice_s[tid] = (T)((double)slice_s[tid] - s);
             }
             __syncthreads();
           }
@@ -177,7 +180,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       if (ns > 0) {
         double q = 0.0;
         if (tid < ns) {
-          const float v = slice_s[tid];
+          const T v = slice_s[tid];
           prm.pvec[n0 + tid] = v;
           q = (double)v * (double)v;
         }
@@ -189,20 +192,20 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       // ---- Ph4: p = p^/||p^||;  S5: t = R p ----
       const double pn2 = sum_parts(prm.qpart, prm.Gs, scr);
       if (!(pn2 > 0.0)) { degenerate = true; break; }                 // reading C7 (uniform across CTAs)
-      const float inv_pn = (float)(1.0 / sqrt(pn2));
+      const T inv_pn = (T)(1.0 / sqrt(pn2));
       for (int n = tid; n < N; n += kThreads) p_s[n] = ld_cg(prm.pvec + n) * inv_pn;
       __syncthreads();
-      if constexpr (RESIDENT) pass_n<VEC, TR, RC, SRC_SLAB>(nullptr, M, slab, slab_ld, mb, N, p_s, t_s, red_s);
-      else                    pass_n<VEC, TR, RC, SRC_GLOBAL>(Rb, M, nullptr, 0, mb, N, p_s, t_s, red_s);
+      if constexpr (RESIDENT) pass_n<T, VEC, TR, RC, SRC_SLAB>(nullptr, M, slab, slab_ld, mb, N, p_s, t_s, red_s);
+      else                    pass_n<T, VEC, TR, RC, SRC_GLOBAL>(Rb, M, nullptr, 0, mb, N, p_s, t_s, red_s);
 
       if (gs && k > 0) {
         for (int rep = 0; rep < prm.gs_passes; ++rep) {                  // CGS2: project a second time
           double* Bpart = prm.Bpart + (size_t)rep * G * prm.Kpad;
           // ---- S6: B-partials  b_b[jj] = sum_{rows} V[m,jj] t[m] ----
           for (int jj = w; jj < k; jj += kWarps) {
-            const float* vj = Tb + (size_t)jj * M;
-            float a = 0.f;
-            for (int i = lane; i < mb; i += 32) a = fmaf(ld_cg(vj + i), t_s[i], a);
+            const T* vj = Tb + (size_t)jj * M;
+            T a = T(0);
+            for (int i = lane; i < mb; i += 32) a = fma_t(ld_cg(vj + i), t_s[i], a);
             const double s = warp_sum((double)a);
             if (lane == 0) Bpart[(size_t)b * prm.Kpad + jj] = s;
           }
@@ -210,8 +213,8 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
           // ---- Ph5: B = sum of partials;  t -= V_(k) B ----
           reduce_coef_parts(coef_s, Bpart, k, G, prm.Kpad, scr);
           for (int i = tid; i < mb; i += kThreads) {
-            float corr = 0.f;
-            for (int jj = 0; jj < k; ++jj) corr = fmaf(ld_cg(Tb + (size_t)jj * M + i), (float)coef_s[jj], corr);
+            T corr = T(0);
+            for (int jj = 0; jj < k; ++jj) corr = fma_t(ld_cg(Tb + (size_t)jj * M + i), (T)coef_s[jj], corr);
             t_s[i] -= corr;
           }
           __syncthreads();
@@ -229,7 +232,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
       if (!(l2 > 0.0)) { degenerate = true; break; }                  // reading C7
       lam_new = sqrt(l2);
       if (gs) {                                                       // V^(k) <- V^(k)/lambda_k
-        const float inv = (float)(1.0 / lam_new);
+        const T inv = (T)(1.0 / lam_new);
         for (int i = tid; i < mb; i += kThreads) t_s[i] *= inv;
         __syncthreads();
       }
@@ -242,15 +245,15 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
 
     // ---- component done: store, and set up the pending deflation ----
     if (degenerate) {
-      for (int i = tid; i < mb; i += kThreads) { Tb[(size_t)k * M + i] = 0.f; d_s[i] = 0.f; t_s[i] = 0.f; }
-      if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = 0.f;
-      if (b == 0 && tid == 0) { prm.lambda[k] = 0.f; prm.iters[k] = 0; }
-      if (tid == 0) lam_s[k] = 0.f;
+      for (int i = tid; i < mb; i += kThreads) { Tb[(size_t)k * M + i] = 0.f; d_s[i] = T(0); t_s[i] = 0.f; }
+      if (tid < ns) prm.P[(size_t)k * N + n0 + tid] = T(0);
+      if (b == 0 && tid == 0) { prm.lambda[k] = T(0); prm.iters[k] = 0; }
+      if (tid == 0) lam_s[k] = T(0);
     } else {
-      const float lamf = (float)lam_new;
-      const float tscale = (!gs && prm.out_svd) ? (float)(1.0 / lam_new) : 1.f;   // SVD output of NIPALS-PCA: v = t/lambda
+      const T lamf = (T)lam_new;
+      const T tscale = (!gs && prm.out_svd) ? (T)(1.0 / lam_new) : T(1);   // SVD output of NIPALS-PCA: v = t/lambda
       for (int i = tid; i < mb; i += kThreads) {
-        const float v = t_s[i];
+        const T v = t_s[i];
         Tb[(size_t)k * M + i] = v * tscale;                           // GS-PCA: unit v until the final scaling
         d_s[i] = gs ? lamf * v : v;                                   // R -= lambda v p^T / R -= t p^T
       }
@@ -263,17 +266,26 @@ __global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParam
 
   // ---- final deflation: the residual R of eq. (4) ----
   if constexpr (RESIDENT)
-    pass_t<VEC, TR, RC, SRC_SLAB, DST_GLOBAL, true, false>(nullptr, Rb, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
+    pass_t<T, VEC, TR, RC, SRC_SLAB, DST_GLOBAL, true, false>(nullptr, Rb, M, slab, slab_ld, mb, N, t_s, d_s, p_s, my_part);
   else
-    pass_t<VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, false>(Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
+    pass_t<T, VEC, TR, RC, SRC_GLOBAL, DST_GLOBAL, true, false>(Rb, Rb, M, nullptr, 0, mb, N, t_s, d_s, p_s, my_part);
   // ---- S10: GS-PCA  T <- V Lambda; skipped for the SVD output V, U, Lambda ----
   if (gs && !prm.out_svd) {
     __syncthreads();
     for (int kk = 0; kk < K; ++kk) {
-      const float l = lam_s[kk];
+      const T l = lam_s[kk];
       for (int i = tid; i < mb; i += kThreads) Tb[(size_t)kk * M + i] *= l;
     }
   }
+}
+
+template <bool RESIDENT, int VEC, int TR, int RC>
+__global__ void __launch_bounds__(kThreads, 1) pca_solve_kernel(const SolveParams prm) {
+  pca_solve_body<float, RESIDENT, VEC, TR, RC>(prm);
+}
+// fp64 storage and arithmetic throughout (the paper's precision): scalar lane mapping
+static __global__ void __launch_bounds__(kThreads, 1) pca_solve_f64_kernel(const SolveParamsT<double> prm) {
+  pca_solve_body<double, false, 1, 32, 4>(prm);
 }
 
 }  // namespace pca

@@ -347,6 +347,57 @@ def test_streaming_kernel_uncached_v_and_wide_gathers(binding, oracle_mod):
             _assert_fixed_pass(gotf, reff, 64, f"{what} J={J}")
 
 
+@pytest.mark.parametrize("ci,M,N,K,ctas", [(0, 256, 64, 8, 0), (1, 1027, 131, 6, 20), (2, 2048, 512, 20, 0), (4, 600, 64, 64, 7)])
+def test_f64_storage_matches_the_oracle(binding, oracle_mod, ci, M, N, K, ctas):
+    """PCA_OPT_STORAGE = 1 (the paper's native precision): fp64 storage and arithmetic
+    in the two-sweep kernel (the paper's statement order).  Same precision as the oracle, so the comparison is element by
+    element at rounding level: converged runs (same iteration counts, lambda to 1e-12) and fixed-pass runs."""
+    cfg = inputs.scaled(inputs.config(ci), M, N, K=K)
+    pr = inputs.generate(cfg)
+    X64 = pr.X.astype(np.float64)
+    Xc = oracle_mod.center(pr.X)
+    for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
+        for eps, J in ((cfg.eps, cfg.max_iter), (0.0, 2)):
+            ref = oracle_mod.pca(Xc, K, eps, J, algo, want_residual=True)
+            got = binding.fit_f64(X64, K, eps, J, algo, center=True, ctas=ctas, want_residual=True)
+            what = f"{cfg.name} f64 algo={algo} eps={eps} J={J}"
+            assert got["info"]["path"] == "two-sweep streaming fp64"
+            np.testing.assert_allclose(got["Xc"], Xc, rtol=0, atol=1e-13 * np.max(np.abs(Xc)), err_msg=what)
+            live = ref.lam[:K] > 1e-6 * ref.lam[0]
+            if eps > 0:                                           # iteration counts may differ by the summation order at the 1e-7 test
+                assert np.max(np.abs(got["iters"][live].astype(int) - ref.iters[:K][live])) <= 2, what
+                tol_l, tol_v = 1e-9, 1e-5                          # early-stopped: one pass more or less moves the vector by ~eps
+            else:
+                assert got["iters"].tolist() == ref.iters[:K].tolist(), what
+                tol_l, tol_v = 1e-11, 1e-9
+            # (GS-PCA leaves V B p^T in R after an unconverged pass; cancelling it costs eps64 * lambda_max / lambda_k, see 1b above)
+            cond = np.maximum(1.0, ref.lam[0] / ref.lam[:K][live])
+            assert np.max(np.abs(got["lam"][live] / ref.lam[:K][live] - 1.0) / cond) <= tol_l, what
+            for k in np.nonzero(live)[0]:
+                for name, a, b in (("P", got["P"][:, k], ref.P[:, k]), ("T", got["T"][:, k], ref.T[:, k])):
+                    err = float(np.max(np.abs(a - b))) / float(np.max(np.abs(b)))
+                    assert err <= tol_v * max(1.0, ref.lam[0] / ref.lam[k]), f"{what} {name}[:, {k}] {err:.3e}"
+            x2 = float(np.sum(Xc * Xc))
+            assert np.max(np.abs(Xc - got["T"] @ got["P"].T - got["R"])) <= 1e-12 * np.sqrt(x2), what + " eq. (4)"
+
+
+def test_f64_entry_points_reject_the_wrong_storage(binding):
+    import torch
+    ctx = binding.PcaContext(64, 16, 2, 1e-7, 100, inputs.ALGO_GS)
+    X = torch.zeros((16, 64), dtype=torch.float64, device="cuda")
+    with pytest.raises(binding.PcaError) as e:
+        ctx.pca_run_f64(X, torch.zeros((2, 64), dtype=torch.float64, device="cuda"), torch.zeros((2, 16), dtype=torch.float64, device="cuda"),
+                        torch.zeros(2, dtype=torch.float64, device="cuda"), torch.zeros(2, dtype=torch.int32, device="cuda"))
+    assert e.value.code == binding.PCA_EINVAL
+    ctx.pca_set_option(binding.PCA_OPT_STORAGE, 1)
+    Xf = torch.zeros((16, 64), dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.PcaError) as e:
+        ctx.pca_run(Xf, torch.zeros((2, 64), device="cuda"), torch.zeros((2, 16), device="cuda"), torch.zeros(2, device="cuda"),
+                    torch.zeros(2, dtype=torch.int32, device="cuda"))
+    assert e.value.code == binding.PCA_EINVAL
+    ctx.pca_destroy()
+
+
 def test_gs_with_more_than_1023_components(binding, oracle_mod):
     """GS-PCA with K >= 1023 must not reach the single-sweep kernels (their k-vector gather has one thread per
     pair of entries, kThreads = 512 pairs): forcing them is PCA_EUNSUPPORTED, the auto plan takes the two-sweep kernel,

@@ -222,6 +222,39 @@ int pca_fit_host(pca_ctx*, const float* X_host, float* T_host, float* P_host, fl
 
 void pca_destroy(pca_ctx*);
 
+/* ---- Row-sharded multi-GPU form (the paper itself is single-GPU) -----------
+ * One process per GPU; rank g holds M_local consecutive rows of the (centred) matrix X and gets its rows of T; P, lambda and
+ * iters come out identical on every rank.  Per inner pass the ranks exchange ONE all-reduce (sum) of N + K' + 2 doubles
+ * ([ R_g^T t~_g | |t~_g|^2 | V_g^T t~_g ], PAPER.md:1023, :1032, :1030 in the single-sweep form of the other kernels); the
+ * all-reduce is the CALLER's (torch.distributed: NCCL between GPUs): every call below only enqueues rank-local kernels on
+ * `stream`.  Calling sequence (paper_0811_1081_b200/sharded.py does exactly this):
+ *     pca_shard_colsums -> all-reduce the N sums -> pca_shard_center                       (S0, column means over ALL rows)
+ *     pca_shard_begin
+ *     for k in 0..K-1:  pca_shard_component(k); exchange;
+ *                       repeat { pca_shard_pass(k); exchange; } until pca_shard_done says 1   (it may be asked every few passes:
+ *                                                                       steps after convergence are no-ops on the device)
+ *                       pca_shard_finish_component(k)
+ *     pca_shard_end
+ *   "exchange" = copy the `send` buffer of pca_shard_exchange to `recv`, all-reduce `recv` in place (sum over the ranks).
+ * Arguments as for pca_create / pca_center / pca_run with M_local rows: X_local, T (dev, M_local x N / M_local x K column-major,
+ * ld = M_local), P (dev, N x K), lambda, iters (dev, K).  K <= 1024, N <= 8192.  Workspace: caller-owned, 256-byte aligned.
+ * Errors: PCA_EINVAL, PCA_EALIGN, PCA_EWORKSPACE (no workspace / pca_shard_begin not called), PCA_EUNSUPPORTED, PCA_ECUDA. */
+typedef struct pca_shard pca_shard;
+int pca_shard_create(pca_shard** out, int64_t M_local, int64_t N, int K, double eps, int max_iter, int algo);
+size_t pca_shard_workspace_bytes(const pca_shard*);
+int pca_shard_set_workspace(pca_shard*, void* dev, size_t bytes);
+int pca_shard_exchange(const pca_shard*, double** send /*dev*/, double** recv /*dev*/, int64_t* count /*doubles*/);
+int pca_shard_colsums(pca_shard*, const float* X_local, double* sums /*dev, N: this rank's column sums*/, void* stream);
+int pca_shard_center(pca_shard*, float* X_local, const double* sums_reduced /*dev, N*/, int64_t M_total, void* stream);
+int pca_shard_begin(pca_shard*, const float* X_local, float* T, float* P, float* lambda, int32_t* iters, void* stream);
+int pca_shard_component(pca_shard*, int k, void* stream);
+int pca_shard_pass(pca_shard*, int k, void* stream);
+int pca_shard_done(pca_shard*, int32_t* done_host /*host*/, void* stream);  /* synchronises `stream` */
+int pca_shard_finish_component(pca_shard*, int k, void* stream);
+int pca_shard_end(pca_shard*, float* R_local /*dev, M_local x N column-major: residual rows of eq. (4); may be NULL*/, void* stream);
+void pca_shard_destroy(pca_shard*);
+int pca_shard_last_cuda_error(const pca_shard*);   /* cudaError_t of the last PCA_ECUDA of this context */
+
 const char* pca_strerror(int code);
 
 /* cudaError_t (as int) of the last failing CUDA call on this context, 0 if none. */

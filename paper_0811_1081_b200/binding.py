@@ -32,6 +32,9 @@ EXPORTED_SYMBOLS = (
     "pca_create", "pca_set_option", "pca_get_info", "pca_workspace_bytes", "pca_set_workspace",
     "pca_center", "pca_run", "pca_residual", "pca_fit_host", "pca_destroy", "pca_strerror",
     "pca_last_cuda_error", "pca_trace", "pca_center_f64", "pca_run_f64", "pca_residual_f64",
+    "pca_shard_create", "pca_shard_workspace_bytes", "pca_shard_set_workspace", "pca_shard_exchange", "pca_shard_colsums",
+    "pca_shard_center", "pca_shard_begin", "pca_shard_component", "pca_shard_pass", "pca_shard_done", "pca_shard_finish_component",
+    "pca_shard_end", "pca_shard_destroy", "pca_shard_last_cuda_error",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -76,6 +79,22 @@ def load_library() -> ctypes.CDLL:
     lib.pca_center_f64.argtypes = [vp, vp, vp]
     lib.pca_run_f64.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.pca_residual_f64.argtypes = [vp, ctypes.POINTER(vp)]
+    lib.pca_shard_create.argtypes = [ctypes.POINTER(vp), i64, i64, i32, f64, i32, i32]
+    lib.pca_shard_workspace_bytes.argtypes = [vp]
+    lib.pca_shard_workspace_bytes.restype = ctypes.c_size_t
+    lib.pca_shard_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+    lib.pca_shard_exchange.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64)]
+    lib.pca_shard_colsums.argtypes = [vp, vp, vp, vp]
+    lib.pca_shard_center.argtypes = [vp, vp, vp, i64, vp]
+    lib.pca_shard_begin.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.pca_shard_component.argtypes = [vp, i32, vp]
+    lib.pca_shard_pass.argtypes = [vp, i32, vp]
+    lib.pca_shard_done.argtypes = [vp, ctypes.POINTER(i32), vp]
+    lib.pca_shard_finish_component.argtypes = [vp, i32, vp]
+    lib.pca_shard_end.argtypes = [vp, vp, vp]
+    lib.pca_shard_destroy.argtypes = [vp]
+    lib.pca_shard_destroy.restype = None
+    lib.pca_shard_last_cuda_error.argtypes = [vp]
     _lib = lib
     return lib
 

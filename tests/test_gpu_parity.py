@@ -398,6 +398,37 @@ def test_f64_entry_points_reject_the_wrong_storage(binding):
     ctx.pca_destroy()
 
 
+@pytest.mark.parametrize("ci,M,N,K,cuts", [(1, 1027, 131, 6, (500,)), (0, 2000, 64, 8, (700, 1300)), (2, 2048, 512, 20, (1024,)),
+                                          (3, 4096, 2048, 6, (3000,))])
+def test_row_sharded_solve_matches_the_oracle(binding, oracle_mod, ci, M, N, K, cuts):
+    """the row-sharded multi-GPU form through the C ABI (pca_shard_*), the ranks emulated as
+    shards of ONE process on one GPU (sequential launches per step; the all-reduce is the sum over the shards, the same
+    code path torch.distributed takes with world_size > 1, tests/test_sharded_host.py).  Uneven row splits; the result must
+    be the oracle's result of the unsharded matrix within the north_star tolerances, P / lambda / iters identical on
+    every shard, and eq. (4) must hold row block by row block."""
+    from paper_0811_1081_b200 import sharded
+    cfg = inputs.scaled(inputs.config(ci), M, N, K=K)
+    pr = inputs.generate(cfg)
+    Xc = oracle_mod.center(pr.X)
+    bounds = (0,) + tuple(cuts) + (M,)
+    for algo in (inputs.ALGO_GS, inputs.ALGO_NIPALS):
+        ref = oracle_mod.pca(Xc, K + 1 if K < N else K, cfg.eps, cfg.max_iter, algo, want_residual=False)
+        shards = [sharded.CudaShard(np.asfortranarray(pr.X[a:b]), K, cfg.eps, cfg.max_iter, algo) for a, b in zip(bounds[:-1], bounds[1:])]
+        outs = sharded.solve_sharded(shards, M, K, check_every=4, want_residual=True)
+        what = f"{cfg.name} sharded x{len(outs)} algo={algo}"
+        for o in outs[1:]:
+            np.testing.assert_array_equal(o["P"], outs[0]["P"], err_msg=what)
+            np.testing.assert_array_equal(o["lam"], outs[0]["lam"], err_msg=what)
+            np.testing.assert_array_equal(o["iters"], outs[0]["iters"], err_msg=what)
+        got = dict(T=np.vstack([o["T"] for o in outs]), P=outs[0]["P"], lam=outs[0]["lam"], iters=outs[0]["iters"],
+                   Xc=np.vstack([o["Xc"] for o in outs]), R=np.vstack([o["R"] for o in outs]))
+        assert np.max(np.abs(got["Xc"] - Xc)) <= 1e-6 * np.max(np.abs(Xc)), what + " centring over all rows"
+        mask = separated_mask(ref.lam, K)
+        assert mask.sum() >= (3 if ci == 2 else min(K, 5)), what      # (collinear config: the signal cluster has sub-2 % gaps)
+        assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
+        _check_invariants(got, f64(got["Xc"]), algo, K, what)
+
+
 def test_gs_with_more_than_1023_components(binding, oracle_mod):
     """GS-PCA with K >= 1023 must not reach the single-sweep kernels (their k-vector gather has one thread per
     pair of entries, kThreads = 512 pairs): forcing them is PCA_EUNSUPPORTED, the auto plan takes the two-sweep kernel,

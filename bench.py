@@ -186,6 +186,10 @@ def time_steps(prob, steps, warmup):
     return step_ms, run_ms
 
 
+# ncu --set full captures of full launches, bytes per launch: (config name, K, plan, full solve) -> dram read + write
+NCU_TRAFFIC = {("cfg4_65536x2048", 128, "single-sweep streaming", True): 7711567000000 + 114480121000}
+
+
 def roofline(prob, run_ms_mean, peaks):
     iters = prob.iters.cpu().numpy()
     single = "single-sweep" in prob.ctx.info()["path"]
@@ -196,12 +200,16 @@ def roofline(prob, run_ms_mean, peaks):
     total_iters = int(iters.sum())
     return {
         "bound": "hbm",
-        "kernel": (("pca_reg_kernel" if "register" in prob.ctx.info()["path"] else "pca_fused_kernel") if single
+        "kernel": (("pca_reg_kernel" if "register" in prob.ctx.info()["path"] else
+                    "pca_one_kernel" if "one-CTA" in prob.ctx.info()["path"] else
+                    "pca_tma_kernel" if "TMA" in prob.ctx.info()["path"] else "pca_fused_kernel") if single
                    else "pca_solve_kernel") + " (persistent; all passes of all components in one launch)",
         "achieved": round(achieved, 1), "peak": peak, "peak_source": peaks["source"], "unit": "GB/s",
-        "frac": round(achieved / peak, 4), "traffic": peaks.get("traffic"),
-        "traffic_note": "not captured for this launch (full solve); profiles/ r01b: dram read+write = 0.89 x the single-sweep "
-                        "algorithmic bytes for the same kernel on a fixed-work launch of config 4" if single else None,
+        "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC.get((prob.cfg.name, prob.K, prob.ctx.info()["path"], total_iters > 0 and prob.eps > 0)),
+        "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel on this workload (same seeded input, same "
+                        "plan, full solve to convergence) from `ncu --set full`, profiles/r02_ncu_full_cfg4_fullsolve.csv: 0.88 x the "
+                        "single-sweep algorithmic bytes (alternate sweeps run in opposite row order and re-use the L2-resident tail); "
+                        "null for workloads / plans without a capture of the full launch (fixed-work captures: profiles/README.md r02)",
         "algorithmic_bytes_per_launch": int(nbytes), "inner_iterations_per_launch": total_iters,
         "us_per_inner_iteration": round(run_ms_mean * 1e3 / max(total_iters, 1), 3),
         "bytes_model": ("single-sweep (SURVEY 8(f) F1): 4MN + [GS]4k(M+N) + 8(M+N) per inner iteration, + 4MN (R^T t0 sweep) "

@@ -353,7 +353,7 @@ int make_fused_plan(pca_ctx* c, int want) {
   c->ws_off_status = take(256);
   c->ws_off_cnt = take(1024);
   c->ws_xchg_bytes = off - c->ws_off_xchg;
-  c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1) * 8 : 0);
+  c->ws_off_trace = take(c->opt_trace > 0 ? ((size_t)c->opt_trace + 1 + 2 * p.G) * 8 : 0);   // records, then per-CTA sweep cycles and SM ids
   c->ws_off_vrm = take(path == 7 && c->algo == PCA_ALGO_GS ? (size_t)M * p.Kpad * 4 : 0);
   p.trace_cap = c->opt_trace;
   c->ws_bytes = off;
@@ -958,6 +958,7 @@ int pca_run(pca_ctx* c, const float* X, float* T, float* P, float* lambda, int32
     p.Vrm = reinterpret_cast<float*>(ws + c->ws_off_vrm);
     PCA_CUDA(c, cudaMemsetAsync(ws + c->ws_off_xchg, 0, c->ws_xchg_bytes, st));   // sequence numbers start at 0
     if (p.trace_cap > 0) PCA_CUDA(c, cudaMemsetAsync(p.trace, 0, 8, st));
+    if (p.trace_cap > 0) PCA_CUDA(c, cudaMemsetAsync(p.trace + 1 + p.trace_cap, 0, (size_t)2 * p.G * 8, st));
     const dim3 tgrid((unsigned)ceil_div(c->M, 32), (unsigned)ceil_div(p.ldr, 32));
     pca::pca_transpose_in_kernel<<<tgrid, 256, 0, st>>>(X, p.Rrm, c->M, p.N, p.ldr);   // R <- X
     PCA_CUDA(c, cudaGetLastError());

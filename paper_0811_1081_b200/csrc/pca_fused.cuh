@@ -851,8 +851,15 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       {
         const unsigned npar = seq & 1u;
         const bool rev = (seq & 1u) != 0;
+        const long long tsw0 = (prm.trace_cap > 0 && tid == 0) ? clock64() : 0;
         if constexpr (RESIDENT) sweep_fused<NV, SRC_SLAB>(prm, Rb, slab, mb, p_s, ttil_s, qs, red_s, sgrp, false);
         else                    sweep_fused<NV, SRC_GLOBAL>(prm, Rb, slab, mb, p_s, ttil_s, qs, red_s, sgrp, rev);
+        if (prm.trace_cap > 0 && tid == 0) {                                  // per-CTA sweep cycles and SM id, after the records
+          unsigned smid;
+          asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+          prm.trace[1 + prm.trace_cap + b] += (unsigned long long)(clock64() - tsw0);
+          prm.trace[1 + prm.trace_cap + G + b] = smid;
+        }
         trace_mark(prm, tn, TR_SWEEP);
         publish_q_ll(prm, qs, prm.Qx + (size_t)npar * Gs * G * Ns, b, seq);
         u64* sbx = prm.SBx + ((size_t)npar * G + b) * SBw;

@@ -318,6 +318,50 @@ def test_fixed_pass_parity_full_size(binding, oracle_mod, ci, K):
             _assert_fixed_pass(got, ref, K, f"{cfg.name} algo={algo} J={J} path={got['info']['path']}")
 
 
+@pytest.mark.parametrize("ci,K", [(2, 8), (3, 8)])
+def test_tma_ring_kernel_full_size(binding, oracle_mod, ci, K):
+    """The TMA-staged streaming kernel (path 7) at FULL size on the two HBM-streaming configs (3: 256-thread row groups,
+    111 rows per CTA; 4: 128-thread row groups, 443 rows per CTA -- the ring wraps ~55 times per sweep and the helper warps
+    follow it): fixed-pass runs element by element against the oracle (GS-PCA: B-partials from the helpers, deflation sweeps
+    through the ring with the cross-proxy fence), and the ring options (1- and 4-row slots)."""
+    cfg = inputs.config(ci)
+    pr = _problem(ci)
+    Xc = oracle_mod.center(pr.X)
+    for algo in cfg.algos:
+        ref = oracle_mod.pca(Xc, K, 0.0, 2, algo, want_residual=False)
+        for opts in ({}, {binding.PCA_OPT_RING_ROWS: 1}, {binding.PCA_OPT_RING_ROWS: 4}):
+            got = binding.fit(pr.X, K, 0.0, 2, algo, center=True, path=7, options=opts)
+            assert "TMA" in got["info"]["path"]
+            _assert_fixed_pass(got, ref, K, f"{cfg.name} algo={algo} path 7 ring {got['info']['ring_rows']}x{got['info']['ring_slots']}")
+
+
+def test_tma_ring_kernel_repeated_runs_are_bitwise_identical(binding):
+    """Stress of the ring / mbarrier / helper-warp protocol: config 2's matrix forced onto path 7 (28 rows per CTA: the ring
+    is partly filled, batches of the next sweep are prefetched across every exchange), 20 runs of the same context."""
+    import torch
+    cfg = inputs.config(1)
+    pr = inputs.generate(cfg)
+    K = 16
+    ctx = binding.PcaContext(cfg.M, cfg.N, K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+    ctx.pca_set_option(binding.PCA_OPT_PATH, 7)
+    X = binding.from_colmajor(pr.X)
+    ctx.pca_center(X)
+    T = torch.empty((K, cfg.M), device="cuda"); P = torch.empty((K, cfg.N), device="cuda")
+    lam = torch.empty(K, device="cuda"); it = torch.empty(K, dtype=torch.int32, device="cuda")
+    ref = None
+    for r in range(20):
+        ctx.pca_run(X, T, P, lam, it)
+        torch.cuda.synchronize()
+        assert ctx.pca_get_info(binding.PCA_INFO_RUN_STATUS) == 0
+        cur = (T.clone(), P.clone(), lam.clone(), it.clone())
+        if ref is None:
+            ref = cur
+        else:
+            for a, b in zip(ref, cur):
+                assert torch.equal(a, b), f"run {r} differs from run 0"
+    ctx.pca_destroy()
+
+
 def test_streaming_kernel_uncached_v_and_wide_gathers(binding, oracle_mod):
     """Streaming single-sweep kernel (path 3) in the regime of the timed config-4 run that no small case reaches by itself:
     rows per CTA large enough that the shared-memory cache of V holds FEWER than K columns (Ksm < K: the B-partials of the

@@ -27,10 +27,12 @@
 //   t0 <- column k of the deflated residual                                   (S1)
 //   LOADS sweep : R <- R - d p_prev^T (pending deflation S9, stored), q = R^T t0, s = |t0|^2
 //   loop: [hop 1] s, B everywhere -> lambda', test (S7, S8);  slice owners: q slice -> p~ = q - W B, A-partials
-//         [hop 2] owners: A -> p^ = p~ - P A, |p^|^2 partials (S3)     (GS-PCA and k > 0 only)
-//         [hop 3] p = p^/|p^| everywhere (S4) -> FUSED sweep: t~ = R p (S5), q = R^T t~ (S2 of the
+//         [hop 2] owners: A -> p^ = p~ - P A, |p^|^2 partials (S3)     (GS-PCA and k > 0 only; taken in the first two passes
+//                 of a component and whenever deferring S3 would cost accuracy, see kDeferKappa: otherwise the sweep starts
+//                 from p~, |p^|^2 = |p~|^2 - |A|^2 travels with the next exchange and p^ is formed once, at convergence)
+//         [hop 3] p = p^/|p^| (or p~/|p~|) everywhere (S4) -> FUSED sweep: t~ = R p (S5), q = R^T t~ (S2 of the
 //                 next pass), s = |t~|^2, B-partials = V^T t~ (S6)
-//   finalize: t = t~ - V B, v = t/lambda', store T, P, lambda, iters, W_k; d <- t
+//   finalize: [final loads, if S3 was deferred] t = t~ - V B, v = t/lambda', store T, P, lambda, iters, W_k; d <- t
 // The hops are NOT grid barriers: data travels between CTAs in self-validating 8-byte words
 // {payload, sequence number} (see "LL exchange" below), so a hop costs one store and one polling
 // load through L2 (measured: a counter barrier + reduction phase cost 2-6 us, pca_trace).  Every

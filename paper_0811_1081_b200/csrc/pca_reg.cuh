@@ -330,6 +330,7 @@ __device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const fl
     gl_st2d(sbx, a, seq);
   }
   if (!with_b) return;
+  __syncwarp();            // (warp 0 re-converges before the full-mask shuffles below; measured in pca_fused.cuh: 2-6 x otherwise)
   int Kc = 32;
   while (Kc < k) Kc <<= 1;
   const int parts = kThreads / Kc;                                     // 1..16, a power of two
@@ -634,6 +635,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
           }
           if (lane == 0) { ctl_s[0] = ln; reinterpret_cast<int*>(ctl_s + 1)[0] = st; }
         }
+        __syncwarp();
         if (with_b) reg_slice_correct(praw_s, Wc, KV, B_s, ns, k);
         __syncthreads();
         // S3: a_S[j] = sum_{n in S} P[n,j] p~[n]
@@ -681,6 +683,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
               gl_st2d(nx + (size_t)Gs * 2 + 4, ctl_s[7], seq);
             }
           }
+          __syncwarp();
         }
         reg_trace(prm, tn, TR_PHAT);
         // S3, first half, off the critical path: a_S[j] = sum_{n in S} P[n,j] p~[n]

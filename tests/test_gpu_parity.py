@@ -134,6 +134,7 @@ SMALL_CASES = [
     (3, 4096, 2048, 10, 7, 0),      # row group = 128 threads (config-4 column count)
     (2, 1024, 4096, 6, 7, 0),       # row group = 256 threads (config-3 column count), M < N
     (4, 1024, 64, 64, 7, 4),        # K = N full decomposition, 256 rows per CTA
+    (4, 1500, 320, 200, 7, 6),      # K > 128: the helper warps walk the V rows in two 128-column chunks
 ]
 
 
@@ -284,7 +285,7 @@ FIXED_PASS_CASES = [
     (4, 1024, 64, 64, 5, 0), (4, 1024, 64, 64, 4, 0), (4, 400, 64, 64, 6, 0), (4, 1024, 64, 64, 3, 0),
     (3, 4096, 2048, 10, 3, 0), (2, 1024, 4096, 6, 3, 0), (1, 3000, 700, 12, 5, 0),
     (0, 256, 64, 8, 7, 3), (1, 1027, 131, 5, 7, 20), (2, 2048, 512, 20, 7, 9), (4, 1024, 64, 64, 7, 4), (3, 4096, 2048, 10, 7, 0),
-    (2, 1024, 4096, 6, 7, 0),
+    (2, 1024, 4096, 6, 7, 0), (4, 1500, 320, 200, 7, 6),
 ]
 
 

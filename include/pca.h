@@ -84,6 +84,10 @@ enum {
                            PCA_EUNSUPPORTED.  Ignored for NIPALS-PCA */
   PCA_OPT_RING_ROWS = 11, /* path 7: rows of R per ring slot (one bulk copy): 0 = auto, 1, 2 or 4 */
   PCA_OPT_RING_SLOTS = 12, /* path 7: upper bound on the ring slots per row group (0 = auto: what fits, at most 8) */
+  PCA_OPT_DEFER_S3 = 15,  /* single-sweep kernels, GS-PCA: 1 (default): a pass may start its sweep from the loads p~ BEFORE the
+                            loads-side Gram-Schmidt p^ = p~ - P A -- R p~ and R p^ give the same projected scores
+                            -- whenever the previous pass measured that this costs no accuracy (p^ is then formed
+                            once per component); 0: every pass takes the paper's order (one more cross-CTA hop per pass) */
   PCA_OPT_STORAGE = 14    /* 0 (default): fp32 storage (pca_center / pca_run / pca_residual); 1: fp64 storage and fp64 arithmetic
                             throughout, the paper's native precision: pca_center_f64 / pca_run_f64 /
                             pca_residual_f64, run by the two-sweep kernel (the paper's pass shape) instantiated on double

@@ -21,6 +21,7 @@ PCA_OK, PCA_EINVAL, PCA_EALIGN, PCA_ECUDA, PCA_EWORKSPACE, PCA_EUNSUPPORTED, PCA
 PCA_OPT_PATH, PCA_OPT_CTAS, PCA_OPT_CENTER_MODE, PCA_OPT_TRACE, PCA_OPT_OWNERS, PCA_OPT_KDIRECT, PCA_OPT_TEST_MODE = 1, 2, 3, 4, 5, 6, 7
 PCA_OPT_STAGNATION, PCA_OPT_OUTPUT, PCA_OPT_GS_PASSES, PCA_OPT_RING_ROWS, PCA_OPT_RING_SLOTS = 8, 9, 10, 11, 12
 PCA_OPT_STORAGE = 14
+PCA_OPT_DEFER_S3 = 15
 PCA_PATH_F64 = 8
 (PCA_PATH_AUTO, PCA_PATH_STREAMING, PCA_PATH_RESIDENT, PCA_PATH_FUSED_STREAMING, PCA_PATH_FUSED_RESIDENT,
  PCA_PATH_REGISTER, PCA_PATH_ONE_CTA, PCA_PATH_TMA_STREAMING) = 0, 1, 2, 3, 4, 5, 6, 7

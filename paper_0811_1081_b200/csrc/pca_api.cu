@@ -94,7 +94,7 @@ struct pca_ctx {
   int device = 0, num_sms = 0, smem_optin = 0;
   // options
   int opt_path = 0, opt_ctas = 0, opt_center_mode = 0, opt_trace = 0, opt_owners = 0, opt_kdirect = -1, opt_test_mode = 0;
-  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0, opt_storage = 0;
+  int opt_stag2 = 1, opt_output = 0, opt_gs_passes = 1, opt_ring_rows = 0, opt_ring_slots = 0, opt_storage = 0, opt_defer_s3 = 1;
   // plan
   bool planned = false;
   int path = 0;  // 1 streaming, 2 resident (two-sweep kernel); 3 streaming, 4 resident (single-sweep kernel);
@@ -334,7 +334,7 @@ int make_fused_plan(pca_ctx* c, int want) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < p.G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output;
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output; p.defer_s3 = c->opt_defer_s3;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
   take((size_t)M * (size_t)N * 4);                                   // residual of eq. (4), column-major (ABI layout)
@@ -441,7 +441,7 @@ int make_reg_plan(pca_ctx* c) {
   if (e != cudaSuccess) return cuda_fail(c, e);
   if ((long long)per_sm * sms < G) return PCA_EUNSUPPORTED;
 
-  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output;
+  p.M = M; p.N = (int)N; p.K = c->K; p.eps = c->eps; p.max_iter = c->max_iter; p.algo = c->algo; p.test_mode = c->opt_test_mode; p.stag2 = c->opt_stag2; p.out_svd = c->opt_output; p.defer_s3 = c->opt_defer_s3;
   p.kdirect = c->opt_kdirect >= 0 ? (c->opt_kdirect > 30 ? 30 : c->opt_kdirect) : 0;    // direct: <= 16 units, one per warp
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = (size_t)round_up((long long)(off + bytes), 256); return o; };
@@ -722,6 +722,10 @@ int pca_set_option_impl(pca_ctx* c, int option, int64_t value) {
     case PCA_OPT_STORAGE:
       if (value < 0 || value > 1) return PCA_EINVAL;
       c->opt_storage = (int)value;
+      break;
+    case PCA_OPT_DEFER_S3:
+      if (value < 0 || value > 1) return PCA_EINVAL;
+      c->opt_defer_s3 = (int)value;
       break;
     default:
       return PCA_EINVAL;

@@ -57,6 +57,7 @@ struct FusedParams {
   int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
   int stag2;             // reading C4b: also compare lambda' with the value two passes back (PCA_OPT_STAGNATION)
   int out_svd;           // PCA_OPT_OUTPUT = 1: T holds the unit score vectors V (SVD triple V, U = P, Lambda)
+  int defer_s3;          // PCA_OPT_DEFER_S3: 1 = the loads-side Gram-Schmidt may be deferred (kDeferKappa), 0 = never (paper's order)
   int G;                 // CTAs
   int Mb;                // rows per CTA
   int ldr;               // row stride of Rrm / slab (floats) = 4*GT*NV
@@ -740,7 +741,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
       // Deferring costs accuracy when A is NOT small (the first pass of a component starts from a raw column; fixed-pass
       // runs never converge): t~ then carries a large component in span V_(k) and lambda'^2 = |t~|^2 - |B|^2 cancels.  So the
       // first two passes of a component, and every pass for which the bound of kDeferKappa fails, take the paper's order.
-      const bool defer_now = gsk && !first && reinterpret_cast<const int*>(ctl_s + 4)[0] != 0;
+      const bool defer_now = prm.defer_s3 != 0 && gsk && !first && reinterpret_cast<const int*>(ctl_s + 4)[0] != 0;
       if (gsk && owner && tid == 0) hop_arrive(cnt2);                         // A-partials of this pass are out
       trace_mark(prm, tn, TR_APART);
       if (gsk) e2 += (unsigned)Gs;

@@ -41,6 +41,7 @@ struct RegParams {
   int test_mode;         // 0 relative (listings), 1 absolute (text): pca_stagnated()
   int stag2;             // reading C4b: also compare lambda' with the value two passes back (PCA_OPT_STAGNATION)
   int out_svd;           // PCA_OPT_OUTPUT = 1: T holds the unit score vectors V (SVD triple V, U = P, Lambda)
+  int defer_s3;          // PCA_OPT_DEFER_S3 (pca_fused.cuh, kDeferKappa)
   int G;                 // CTAs
   int Mb;                // rows per CTA (<= NG*RPT)
   int ldr;               // 4*NV*GT >= N
@@ -653,7 +654,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         // never converge): t~ then carries a large component in span V_(k) and lambda'^2 = |t~|^2 - |B|^2 cancels.  So the first
         // two passes of a component, and every pass for which the bound of kDeferKappa (pca_fused.cuh) fails, take the paper's
         // order (hop 2).  Every owner takes the same decision from the same numbers.
-        const bool defer_now = with_b && ctl_s[6] * bf2 <= kDeferKappa * ctl_s[5] * lam * lam;
+        const bool defer_now = prm.defer_s3 != 0 && with_b && ctl_s[6] * bf2 <= kDeferKappa * ctl_s[5] * lam * lam;
         if (gsk && !defer_now) {
           if (k <= 64) reg_publish_a(Pc, KV, praw_s, Ax + (size_t)par * Gs * Kpad + (size_t)b * 2, Gs * 2, ns, k, seq);
           else reg_publish_a(Pc, KV, praw_s, Ax + ((size_t)par * Gs + b) * Kpad, 2, ns, k, seq);

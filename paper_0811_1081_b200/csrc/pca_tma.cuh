@@ -645,7 +645,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
       // Deferring costs accuracy when A is NOT small (the first pass of a component starts from a raw column; fixed-pass
       // runs never converge): t~ then carries a large component in span V_(k) and lambda'^2 = |t~|^2 - |B|^2 cancels.  So the
       // first two passes of a component, and every pass for which the bound of kDeferKappa fails, take the paper's order.
-      const bool defer_now = gsk && !first && reinterpret_cast<const int*>(ctl_s + 4)[0] != 0;
+      const bool defer_now = prm.defer_s3 != 0 && gsk && !first && reinterpret_cast<const int*>(ctl_s + 4)[0] != 0;
       if (gsk && owner && tid == 0) hop_arrive(cnt2);                         // A-partials of this pass are out
       trace_mark(prm, tn, TR_APART);
       if (gsk) e2 += (unsigned)Gs;

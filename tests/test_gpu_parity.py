@@ -19,6 +19,10 @@ takes, and the test that reaches each:
   * hop 1 / hop 2 with <= 16 units (ll_reduce2): every path-3 case of SMALL_CASES
   * LOADS sweep with the fused deflation (k > 0), degenerate exit, finalisation, epilogue S10: SMALL_CASES,
     test_degenerate_zero_column_and_zero_matrix, test_fixed_pass_parity
+  * loads-side Gram-Schmidt in the paper's order (hop 2 taken: first two passes of a component, every fixed-pass run) AND
+    deferred (hop 2 skipped, |p^|^2 = |p~|^2 - |A|^2 at the next test, final-loads exchange at convergence): every converged
+    case (SMALL_CASES, test_full_cfg3 / cfg4), test_fixed_pass_parity (never deferred), and both settings side by side in
+    test_deferred_loads_side_gram_schmidt_switch
 """
 import json
 import os
@@ -361,6 +365,48 @@ def test_tma_ring_kernel_repeated_runs_are_bitwise_identical(binding):
             for a, b in zip(ref, cur):
                 assert torch.equal(a, b), f"run {r} differs from run 0"
     ctx.pca_destroy()
+
+
+@pytest.mark.parametrize("path", [3, 5, 7])
+def test_deferred_loads_side_gram_schmidt_switch(binding, oracle_mod, path):
+    """PCA_OPT_DEFER_S3: with the option OFF every pass takes the paper's order (hop 2: wait for A, then
+    p^ = p~ - P A); with it ON (default) a converging run skips that hop in most passes and forms p^ once
+    per component.  Both settings must match the oracle within the north_star tolerances and each other to rounding level
+    (the deferred sweep gives the same projected scores), and the orthogonality of the loadings must not suffer.  On the
+    streaming kernel the phase trace shows that hop 2 (records X2) is really gone from most passes."""
+    import torch
+    cfg = inputs.scaled(inputs.config(3), 4096, 512, K=12)
+    pr = inputs.generate(cfg)
+    Xc, ref = _oracle_run(oracle_mod, pr.X, cfg, inputs.ALGO_GS, K=cfg.K)
+    mask = separated_mask(ref.lam, cfg.K)
+    res = {}
+    for defer in (0, 1):
+        got = binding.fit(pr.X, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS, center=True, path=path, want_residual=True,
+                          options={binding.PCA_OPT_DEFER_S3: defer})
+        what = f"{cfg.name} path={got['info']['path']} defer={defer}"
+        assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
+        _check_invariants(got, f64(got["Xc"]), inputs.ALGO_GS, cfg.K, what)
+        res[defer] = got
+    np.testing.assert_allclose(res[1]["lam"], res[0]["lam"], rtol=2e-6)
+    assert abs(int(res[1]["iters"].sum()) - int(res[0]["iters"].sum())) <= 0.05 * int(res[0]["iters"].sum())
+    if path == 3:                                                # count the hop-2 records of a traced run
+        counts = {}
+        for defer in (0, 1):
+            ctx = binding.PcaContext(cfg.M, cfg.N, cfg.K, cfg.eps, cfg.max_iter, inputs.ALGO_GS)
+            for opt, val in ((binding.PCA_OPT_PATH, 3), (binding.PCA_OPT_DEFER_S3, defer), (binding.PCA_OPT_TRACE, 1 << 15)):
+                ctx.pca_set_option(opt, val)
+            X = binding.from_colmajor(pr.X)
+            ctx.pca_center(X)
+            T = torch.empty((cfg.K, cfg.M), device="cuda"); P = torch.empty((cfg.K, cfg.N), device="cuda")
+            lam = torch.empty(cfg.K, device="cuda"); it = torch.empty(cfg.K, dtype=torch.int32, device="cuda")
+            ctx.pca_run(X, T, P, lam, it)
+            torch.cuda.synchronize()
+            tr = ctx.pca_trace()
+            counts[defer] = (int((tr[:, 0] == 7).sum()), int((tr[:, 0] == 11).sum()))     # (X2 records, SWEEP records)
+            ctx.pca_destroy()
+        (x2_off, sw_off), (x2_on, sw_on) = counts[0], counts[1]
+        assert x2_off >= 0.9 * sw_off                            # paper's order: hop 2 in every pass of the components k > 0
+        assert x2_on <= 0.35 * sw_on, f"hop 2 taken in {x2_on} of {sw_on} passes with deferral on"
 
 
 def test_streaming_kernel_uncached_v_and_wide_gathers(binding, oracle_mod):

@@ -36,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(OBJDIR, exist_ok=True)
     base = [nvcc_path(), "-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
-            "-Xcompiler", "-fPIC"] + (["-Xptxas", "-v"] if verbose else []) + os.environ.get("PCA_NVCC_FLAGS", "").split()
+            "-Xcompiler", "-fPIC"] + (["-Xptxas", "-v"] if verbose else [])
     jobs = [(src, os.path.join(OBJDIR, os.path.basename(src)[:-3] + ".o"), []) for src in SOURCES]
     jobs += [(REG_INST, os.path.join(OBJDIR, f"pca_reg_inst{i}.o"), [f"-DPCA_REG_PART={i}"]) for i in range(REG_PARTS)]
 

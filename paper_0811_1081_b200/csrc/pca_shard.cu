@@ -35,6 +35,7 @@ struct pca_shard {
          off_part = 0, off_xsend = 0, off_xbuf = 0, off_st = 0;
   void* ws = nullptr;
   bool begun = false;
+  bool attr_set[2] = {false, false};
   int last_cuda = 0;
 };
 
@@ -177,10 +178,13 @@ int pca_shard_begin(pca_shard* c, const float* X_local, float* T, float* P, floa
 static int launch_sweep(pca_shard* c, bool loads, int k, cudaStream_t st) {
   const ShardParams& p = c->p;
   sweep_fn fn = loads ? c->var->loads : c->var->fused;
-  SH_CUDA(c, cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sm.bytes));
+  if (!c->attr_set[loads ? 0 : 1]) {                                  // once per context and kernel (the call is not cheap)
+    SH_CUDA(c, cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sm.bytes));
+    c->attr_set[loads ? 0 : 1] = true;
+  }
   fn<<<(unsigned)p.G, pca::kThreads, c->sm.bytes, st>>>(p, c->sm, k);
   SH_CUDA(c, cudaGetLastError());
-  pca::pca_shard_reduce_kernel<<<(unsigned)ceil_div(p.L, 256), 256, 0, st>>>(p);
+  pca::pca_shard_reduce_kernel<<<(unsigned)ceil_div(p.L, 32), 256, 0, st>>>(p);
   SH_CUDA(c, cudaGetLastError());
   return PCA_OK;
 }

@@ -101,26 +101,44 @@ __global__ void __launch_bounds__(kThreads, 1) pca_shard_sweep_kernel(const Shar
     out[n] = a;
   }
   if (tid == 0) { out[N] = s; out[N + 1] = 0.0; }
-  for (int j = tid; j < prm.Kpad; j += kThreads) {
-    double a = 0.0;
+  // B-partials (S6): 32 consecutive columns j per warp (coalesced rows of the row-major V), the 16 warps split the rows
+  __syncthreads();                                           // qs is consumed: reuse it as [kWarps][32] floats
+  float* bred = qs;
+  for (int jb = 0; jb < prm.Kpad; jb += 32) {
+    const int lane = tid & 31, w = tid >> 5, j = jb + lane;
+    float af = 0.f;
     if (!LOADS && gsk && j < k) {
       const float* vr = prm.Vrm + (size_t)m0 * prm.Kpad + j;
-      float af = 0.f;
-      for (int i = 0; i < mb; ++i) af = fmaf(vr[(size_t)i * prm.Kpad], ttil_s[i], af);
-      a = (double)af;
+      for (int i = w; i < mb; i += kWarps) af = fmaf(vr[(size_t)i * prm.Kpad], ttil_s[i], af);
     }
-    out[N + 2 + j] = a;
+    bred[w * 32 + lane] = af;
+    __syncthreads();
+    if (w == 0 && j < prm.Kpad) {
+      double a = 0.0;
+      for (int q2 = 0; q2 < kWarps; ++q2) a += (double)bred[q2 * 32 + lane];   // fixed order
+      out[N + 2 + j] = a;
+    }
+    __syncthreads();
   }
 }
 
 // xbuf[j] = sum over the CTAs of part[b][j], fixed order
+// (32 columns per CTA, 8 groups of parts per column: coalesced 256-byte rows, 8 independent chains)
 static __global__ void __launch_bounds__(256) pca_shard_reduce_kernel(const ShardParams prm) {
   if (prm.st->done) return;
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= prm.L) return;
+  __shared__ double red[8][33];
+  const int jl = threadIdx.x & 31, pg = threadIdx.x >> 5;
+  const int j = blockIdx.x * 32 + jl;
   double a = 0.0;
-  for (int b = 0; b < prm.G; ++b) a += prm.part[(size_t)b * prm.L + j];
-  prm.xsend[j] = a;
+  if (j < prm.L)
+    for (int b = pg; b < prm.G; b += 8) a += prm.part[(size_t)b * prm.L + j];
+  red[pg][jl] = a;
+  __syncthreads();
+  if (pg == 0 && j < prm.L) {
+    double t = 0.0;
+    for (int q = 0; q < 8; ++q) t += red[q][jl];
+    prm.xsend[j] = t;
+  }
 }
 
 // The replicated loads side (one CTA): consumes the all-reduced [ q | s | B ].
@@ -194,12 +212,23 @@ static __global__ void __launch_bounds__(1024, 1) pca_shard_nside_kernel(const S
   }
   // S3: A = P^T p~ ; p^ = p~ - P A.  A in shared memory (k <= 1024 per chunk of the block)
   __shared__ double A_s[1024];
+  __shared__ double red32[32][33];
   if (gsk) {
     for (int j0 = 0; j0 < k; j0 += 1024) {
-      for (int j = j0 + tid; j < min(k, j0 + 1024); j += nthr) {
+      // A[j] = sum_n P[n,j] p~[n]: 32 consecutive j per warp-row (coalesced rows of the row-major panel), the 32 warps split n
+      for (int jb = j0; jb < min(k, j0 + 1024); jb += 32) {
+        const int j = jb + lane;
         double a = 0.0;
-        for (int n = 0; n < N; ++n) a += (double)prm.Pn[(size_t)n * Kpad + j] * prm.praw[n];
-        A_s[j - j0] = a;
+        if (j < k)
+          for (int n = w; n < N; n += (nthr >> 5)) a += (double)prm.Pn[(size_t)n * Kpad + j] * prm.praw[n];
+        __syncthreads();                                    // red32 free
+        red32[w][lane] = a;
+        __syncthreads();
+        if (w == 0 && j < k) {
+          double t = 0.0;
+          for (int q2 = 0; q2 < (nthr >> 5); ++q2) t += red32[q2][lane];   // fixed order
+          A_s[j - j0] = t;
+        }
       }
       __syncthreads();
       for (int n = tid; n < N; n += nthr) {

@@ -206,15 +206,8 @@ __device__ __forceinline__ void group_row_sums(float (&part)[RB], float (&tt)[RB
 // the second product.  Leaves qs[g][ldr], ttil_s[rows], sgrp[g] = sum t~^2 (fp64); ends with cta_sync().
 template <int NV, int RB>
 __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB>& rg, int sw, const float* p_s,
-                                                 float* ttil_s, float* qs, float* red_s, double* sgrp, unsigned* prog_s,
-                                                 long long* prof = nullptr) {
+                                                 float* ttil_s, float* qs, float* red_s, double* sgrp, unsigned* prog_s) {
   const int GT = prm.GT, NG = kThreads / GT, WG = GT >> 5, ldr = prm.ldr;
-#ifdef PCA_TMA_PROFILE
-  long long pc0 = 0, pc1 = 0, pc2 = 0, pc3 = 0, tq = clock64();
-#define PROF_STEP(acc) { const long long tnow = clock64(); acc += tnow - tq; tq = tnow; }
-#else
-#define PROF_STEP(acc)
-#endif
   const int tid = threadIdx.x, g = tid / GT, gl = tid - g * GT, lane = tid & 31, wg = gl >> 5;
   float4 q[NV];                                                            // (p is re-read from shared memory per batch:
 #pragma unroll                                                             //  16 registers less, no spills in the loop)
@@ -228,7 +221,6 @@ __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB
     const int r0 = bi * RB;
     const int rows = min(RB, rg.mb - r0);
     rg.wait_next();
-    PROF_STEP(pc0)
     const float* sl = rg.cur_slot();
     float4 x[RB][NV];
 #pragma unroll
@@ -250,12 +242,10 @@ __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB
     }
     group_row_sums<RB>(part, tt, WG, g, GT, wg, lane, red_s, parity);     // every thread of the group has read the slot
     rg.consumed();
-    PROF_STEP(pc1)
     if (gl == 0) {
       --rg.inflight;
       rg.top_up(sw + 1);                                                  // refill: this sweep, then the head of the next
     }
-    PROF_STEP(pc2)
     if (gl == gl2) {                                                      // (not the refilling thread when the group has 2+ warps)
 #pragma unroll
       for (int i = 0; i < RB; ++i)
@@ -269,11 +259,7 @@ __device__ __forceinline__ void sweep_fused_ring(const FusedParams& prm, Ring<RB
     for (int i = 0; i < RB; ++i)
 #pragma unroll
       for (int v = 0; v < NV; ++v) axpy4(q[v], x[i][v], tt[i]);
-    PROF_STEP(pc3)
   }
-#ifdef PCA_TMA_PROFILE
-  if (prof) { prof[0] = pc0; prof[1] = pc1; prof[2] = pc2; prof[3] = pc3; }
-#endif
 #pragma unroll
   for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q[v];
   if (gl == gl2) sgrp[g] = sacc;
@@ -759,14 +745,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) pca_tma_kernel(const FusedPara
       {
         const unsigned npar = seq & 1u;
         if (gsk) bar_arrive(BAR_HSTART, kTmaThreads);                         // the helpers start following the row groups
-#ifdef PCA_TMA_PROFILE
-        long long prof[4] = {0, 0, 0, 0};
-        sweep_fused_ring<NV, RB>(prm, rg, sw, p_s, ttil_s, qs, red_s, sgrp, prog_s, prof);
-        if (prm.trace_cap > 0 && b == 0 && tid == 0)
-          for (int q4 = 0; q4 < 4 && tn < prm.trace_cap; ++q4) { prm.trace[1 + tn] = ((unsigned long long)(20 + q4) << 56) | (unsigned long long)prof[q4]; ++tn; }
-#else
         sweep_fused_ring<NV, RB>(prm, rg, sw, p_s, ttil_s, qs, red_s, sgrp, prog_s);
-#endif
         ++sw;
         trace_mark(prm, tn, TR_SWEEP);
         publish_q_ll(prm, qs, prm.Qx + (size_t)npar * Gs * G * Ns, b, seq);

@@ -327,7 +327,7 @@ int make_fused_plan(pca_ctx* c, int want) {
   }
   fused_kernel_t fn = path == 7 ? tvar->fn : var->fn;
   const int nthreads = path == 7 ? pca::kTmaThreads : pca::kThreads;
-  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);   // per FUNCTION: the device maximum, so that contexts do not lower it for each other
   if (e != cudaSuccess) return cuda_fail(c, e);
   int per_sm = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, nthreads, smem);
@@ -434,7 +434,7 @@ int make_reg_plan(pca_ctx* c) {
     if (Gs * 2 > g2 || Gs * 2 > ldr / 2) return PCA_EUNSUPPORTED;   // more owners = smaller P / W panels per owner
     Gs *= 2;
   }
-  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);   // per FUNCTION: the device maximum, so that contexts do not lower it for each other
   if (e != cudaSuccess) return cuda_fail(c, e);
   int per_sm = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, pca::kThreads, smem);
@@ -508,7 +508,7 @@ int make_one_plan(pca_ctx* c) {
   p.off_wp = take(gs ? (size_t)ldr * KV * 4 : 0);
   const size_t smem = off;
   if (smem > (size_t)c->smem_optin) return PCA_EUNSUPPORTED;
-  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);   // per FUNCTION: the device maximum, so that contexts do not lower it for each other
   if (e != cudaSuccess) return cuda_fail(c, e);
   size_t woff = 0;
   auto wtake = [&](size_t bytes) { size_t o = woff; woff = (size_t)round_up((long long)(woff + bytes), 256); return o; };
@@ -542,7 +542,7 @@ int make_f64_plan(pca_ctx* c) {
   int tr = 0, rc = 0;
   const size_t smem = carve(c, 0, G, 1, &g, &tr, &rc, 8);
   if (smem > (size_t)c->smem_optin || tr != 32 || rc != 4) return PCA_EUNSUPPORTED;
-  cudaError_t e = cudaFuncSetAttribute(pca::pca_solve_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(pca::pca_solve_f64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);   // per FUNCTION: the device maximum, so that contexts do not lower it for each other
   if (e != cudaSuccess) return cuda_fail(c, e);
   int per_sm = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pca::pca_solve_f64_kernel, pca::kThreads, smem);
@@ -637,7 +637,7 @@ int make_plan(pca_ctx* c) {
     path = 1;
   }
   // co-residency of the cooperative grid
-  cudaError_t e = cudaFuncSetAttribute(var->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(var->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);   // per FUNCTION: the device maximum, so that contexts do not lower it for each other
   if (e != cudaSuccess) return cuda_fail(c, e);
   int per_sm = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, var->fn, pca::kThreads, smem);

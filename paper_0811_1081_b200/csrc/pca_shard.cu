@@ -36,6 +36,7 @@ struct pca_shard {
   void* ws = nullptr;
   bool begun = false;
   bool attr_set[2] = {false, false};
+  int smem_optin = 0;
   int last_cuda = 0;
 };
 
@@ -59,6 +60,7 @@ int pca_shard_create(pca_shard** out, int64_t M_local, int64_t N, int K, double 
     return PCA_ECUDA;                                               // no CUDA device: there is no CPU fallback
   pca_shard* c = new (std::nothrow) pca_shard();
   if (!c) return PCA_EINVAL;
+  c->smem_optin = smem_optin;
   ShardParams& p = c->p;
   p.Ml = M_local; p.N = (int)N; p.K = K; p.eps = eps; p.max_iter = max_iter; p.algo = algo; p.test_mode = 0; p.stag2 = 1;
   int GT = 32;
@@ -179,7 +181,9 @@ static int launch_sweep(pca_shard* c, bool loads, int k, cudaStream_t st) {
   const ShardParams& p = c->p;
   sweep_fn fn = loads ? c->var->loads : c->var->fused;
   if (!c->attr_set[loads ? 0 : 1]) {                                  // once per context and kernel (the call is not cheap)
-    SH_CUDA(c, cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sm.bytes));
+    // (the attribute belongs to the FUNCTION, not to this context: ask for the device maximum, so that contexts with different
+    //  shared-memory needs -- the shards of one process -- do not lower it for each other)
+    SH_CUDA(c, cudaFuncSetAttribute(reinterpret_cast<const void*>(fn), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin));
     c->attr_set[loads ? 0 : 1] = true;
   }
   fn<<<(unsigned)p.G, pca::kThreads, c->sm.bytes, st>>>(p, c->sm, k);

@@ -472,6 +472,47 @@ def test_f64_storage_matches_the_oracle(binding, oracle_mod, ci, M, N, K, ctas):
             assert np.max(np.abs(Xc - got["T"] @ got["P"].T - got["R"])) <= 1e-12 * np.sqrt(x2), what + " eq. (4)"
 
 
+def test_two_contexts_sharing_a_kernel_variant(binding, oracle_mod):
+    """Two live contexts whose plans pick the same kernel instantiation with different shared-memory needs: the dynamic
+    shared-memory attribute belongs to the function, so the second plan must not lower it under the first context's need."""
+    import torch
+    big = inputs.scaled(inputs.config(3), 40000, 2048, K=2)         # path 3, 271 rows per CTA
+    small = inputs.scaled(inputs.config(3), 3000, 2048, K=2)        # same <NV = 4> streaming instantiation, 21 rows per CTA
+    ctxs = []
+    for cfg in (big, small):
+        ctx = binding.PcaContext(cfg.M, cfg.N, cfg.K, 0.0, 2, inputs.ALGO_GS)
+        ctx.pca_set_option(binding.PCA_OPT_PATH, 3)
+        ctxs.append((cfg, ctx))
+    assert ctxs[0][1].pca_get_info(binding.PCA_INFO_SMEM_BYTES) > ctxs[1][1].pca_get_info(binding.PCA_INFO_SMEM_BYTES)
+    for cfg, ctx in ctxs:                                           # the big one runs AFTER the small one was planned
+        pr = inputs.generate(cfg)
+        X = binding.from_colmajor(pr.X)
+        ctx.pca_center(X)
+        T = torch.empty((cfg.K, cfg.M), device="cuda"); P = torch.empty((cfg.K, cfg.N), device="cuda")
+        lam = torch.empty(cfg.K, device="cuda"); it = torch.empty(cfg.K, dtype=torch.int32, device="cuda")
+        ctx.pca_run(X, T, P, lam, it)
+        torch.cuda.synchronize()
+        ref = oracle_mod.pca(oracle_mod.center(pr.X), cfg.K, 0.0, 2, inputs.ALGO_GS, want_residual=False)
+        np.testing.assert_allclose(lam.cpu().numpy(), ref.lam[:cfg.K], rtol=2e-5)
+    for _, ctx in ctxs:
+        ctx.pca_destroy()
+
+
+def test_f64_storage_with_cgs2(binding, oracle_mod):
+    """fp64 storage together with PCA_OPT_GS_PASSES = 2 (CGS2) against the oracle's gs_passes = 2 mode."""
+    cfg = inputs.scaled(inputs.config(1), 700, 90, K=6)
+    pr = inputs.generate(cfg)
+    Xc = oracle_mod.center(pr.X)
+    ref = oracle_mod.pca(Xc, cfg.K, 0.0, 3, inputs.ALGO_GS, want_residual=False, gs_passes=2)
+    got = binding.fit_f64(pr.X.astype(np.float64), cfg.K, 0.0, 3, inputs.ALGO_GS, center=True, options={binding.PCA_OPT_GS_PASSES: 2})
+    assert got["iters"].tolist() == ref.iters[:cfg.K].tolist()
+    np.testing.assert_allclose(got["lam"], ref.lam[:cfg.K], rtol=1e-10)
+    np.testing.assert_allclose(got["P"], ref.P[:, :cfg.K], atol=1e-9)
+    np.testing.assert_allclose(got["T"], ref.T[:, :cfg.K], atol=1e-9 * np.max(np.abs(ref.T)))
+    Pd = got["P"]
+    assert np.max(np.abs(Pd.T @ Pd - np.eye(cfg.K))) <= 1e-13
+
+
 def test_f64_entry_points_reject_the_wrong_storage(binding):
     import torch
     ctx = binding.PcaContext(64, 16, 2, 1e-7, 100, inputs.ALGO_GS)
@@ -490,7 +531,7 @@ def test_f64_entry_points_reject_the_wrong_storage(binding):
 
 
 @pytest.mark.parametrize("ci,M,N,K,cuts", [(1, 1027, 131, 6, (500,)), (0, 2000, 64, 8, (700, 1300)), (2, 2048, 512, 20, (1024,)),
-                                          (3, 4096, 2048, 6, (3000,))])
+                                          (3, 4096, 2048, 6, (3000,)), (0, 200, 64, 8, (150,)), (4, 600, 64, 64, (300,))])
 def test_row_sharded_solve_matches_the_oracle(binding, oracle_mod, ci, M, N, K, cuts):
     """the row-sharded multi-GPU form through the C ABI (pca_shard_*), the ranks emulated as
     shards of ONE process on one GPU (sequential launches per step; the all-reduce is the sum over the shards, the same
@@ -515,7 +556,7 @@ def test_row_sharded_solve_matches_the_oracle(binding, oracle_mod, ci, M, N, K, 
                    Xc=np.vstack([o["Xc"] for o in outs]), R=np.vstack([o["R"] for o in outs]))
         assert np.max(np.abs(got["Xc"] - Xc)) <= 1e-6 * np.max(np.abs(Xc)), what + " centring over all rows"
         mask = separated_mask(ref.lam, K)
-        assert mask.sum() >= (3 if ci == 2 else min(K, 5)), what      # (collinear config: the signal cluster has sub-2 % gaps)
+        assert mask.sum() >= (3 if ci == 2 else 0 if ci == 4 else min(K, 5)), what   # (collinear config: sub-2 % gaps; config 5: none separated)
         assert_separated_parity(got["P"], got["T"], got["lam"], ref.P, ref.T, ref.lam, mask, what)
         _check_invariants(got, f64(got["Xc"]), algo, K, what)
 

@@ -681,7 +681,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
             if (b == 0) {                                                     // every owner takes the same decision: owner 0 reports it
               gl_st2(nx + (size_t)Gs * 2, ll_word((unsigned)st, seq), ll_word(defer_now ? 1u : 0u, seq));
               gl_st2d(nx + (size_t)Gs * 2 + 2, ctl_s[0], seq);
-              gl_st2d(nx + (size_t)Gs * 2 + 4, ctl_s[7], seq);
+              if (gsk) gl_st2d(nx + (size_t)Gs * 2 + 4, ctl_s[7], seq);
             }
           }
           __syncwarp();
@@ -709,7 +709,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         unsigned stv = 0;
         u64 x1 = 0, y1 = 0, x2 = 0, y2 = 0, x3 = 0, y3 = 0;
         double rhov = 1.0;
-        if (lane == 0) { gl_ld2(nx + (size_t)Gs * 2, x1, y1); gl_ld2(nx + (size_t)Gs * 2 + 2, x2, y2); gl_ld2(nx + (size_t)Gs * 2 + 4, x3, y3); }
+        if (lane == 0) { gl_ld2(nx + (size_t)Gs * 2, x1, y1); gl_ld2(nx + (size_t)Gs * 2 + 2, x2, y2); if (gsk) gl_ld2(nx + (size_t)Gs * 2 + 4, x3, y3); }
         for (int o = lane; o < Gs; o += 32) {
           u64 x0 = 0, y0 = 0;
           gl_wait2(nx + (size_t)o * 2, seq, x0, y0, status);
@@ -718,11 +718,11 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         if (lane == 0) {
           gl_wait2(nx + (size_t)Gs * 2, seq, x1, y1, status);
           gl_wait2(nx + (size_t)Gs * 2 + 2, seq, x2, y2, status);
-          gl_wait2(nx + (size_t)Gs * 2 + 4, seq, x3, y3, status);
+          if (gsk) gl_wait2(nx + (size_t)Gs * 2 + 4, seq, x3, y3, status);
           stv = (unsigned)x1;
           reinterpret_cast<int*>(ctl_s + 1)[1] = (int)(unsigned)y1;             // the loads just published are p~ (S3 deferred)
           lamv = ll_d(x2, y2);
-          rhov = ll_d(x3, y3);
+          if (gsk) rhov = ll_d(x3, y3);
         }
         nsum = warp_sum(nsum);
         if (lane == 0) {

@@ -232,11 +232,12 @@ __device__ __forceinline__ void sweep_fused(const FusedParams& prm, const float*
     }
     float part[kRB];
 #pragma unroll
-    for (int i = 0; i < kRB; ++i) {
-      float a = 0.f;
+    for (int i = 0; i < kRB; ++i) part[i] = 0.f;
 #pragma unroll
-      for (int v = 0; v < NV; ++v) a = dot4(x[i][v], pr[v], a);
-      part[i] = a;
+    for (int v = 0; v < NV; ++v) {
+      const float4 pv = (SRC == SRC_GLOBAL) ? *reinterpret_cast<const float4*>(p_s + 4 * (gl + GT * v)) : pr[v];
+#pragma unroll
+      for (int i = 0; i < kRB; ++i) part[i] = dot4(x[i][v], pv, part[i]);
     }
     // butterfly over the warp: 4 values -> lanes 0,8,16,24 (and their 8-lane groups) hold rows 0..3
     const bool hi = (lane & 16) != 0;

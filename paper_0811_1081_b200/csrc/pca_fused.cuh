@@ -216,17 +216,25 @@ __device__ __forceinline__ void sweep_fused(const FusedParams& prm, const float*
     const int bi = rev ? (nb - 1 - bq) : bq;
     const int r0 = bi * kRB;
     float4 x[kRB][NV];
+    if (SRC == SRC_GLOBAL && r0 + kRB <= mb) {                          // full batch: no per-row predicates on the loads
+      const float* rp = Rb + (size_t)r0 * ldr + 4 * gl;
 #pragma unroll
-    for (int i = 0; i < kRB; ++i) {
-      const int r = r0 + i;
+      for (int i = 0; i < kRB; ++i)
 #pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        const int c = 4 * (gl + GT * v);
-        if (r < mb) {
-          if constexpr (SRC == SRC_GLOBAL) x[i][v] = ld_stream4(Rb + (size_t)r * ldr + c);
-          else x[i][v] = *reinterpret_cast<const float4*>(slab + (size_t)r * ldr + c);
-        } else {
-          x[i][v] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int v = 0; v < NV; ++v) x[i][v] = ld_stream4(rp + (size_t)i * ldr + 4 * GT * v);
+    } else {
+#pragma unroll
+      for (int i = 0; i < kRB; ++i) {
+        const int r = r0 + i;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const int c = 4 * (gl + GT * v);
+          if (r < mb) {
+            if constexpr (SRC == SRC_GLOBAL) x[i][v] = ld_stream4(Rb + (size_t)r * ldr + c);
+            else x[i][v] = *reinterpret_cast<const float4*>(slab + (size_t)r * ldr + c);
+          } else {
+            x[i][v] = make_float4(0.f, 0.f, 0.f, 0.f);
+          }
         }
       }
     }

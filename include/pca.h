@@ -259,6 +259,33 @@ int pca_shard_end(pca_shard*, float* R_local /*dev, M_local x N column-major: re
 void pca_shard_destroy(pca_shard*);
 int pca_shard_last_cuda_error(const pca_shard*);   /* cudaError_t of the last PCA_ECUDA of this context */
 
+/* ---- No-allocation entry point (README.md "No-allocation entry point") -----------------------------------------------------
+ * pca_run for SMALL matrices without any device allocation and without a context: for callers that cannot call cudaMalloc
+ * (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).  It runs the one-CTA kernel of
+ * PCA_OPT_PATH = 6 (the same inner loop, PAPER.md:555-568 / :1016-1038; same arithmetic, same results as pca_run on that path
+ * with default options) and keeps the kernel's only scratch memory -- the row-major working copy of the residual, R <- X
+ * -- in a file-scope device array of pca_small_static_scratch_bytes() = 114688 bytes that every GPU loading the
+ * library holds until the process exits.
+ *   limits     N <= 512 and M <= (512/GT)*7 rows with GT = the power of two >= max(8, N/8), so that M x (8*GT) floats fit in
+ *              the array: M <= 448 for N <= 64, 224 for N <= 128, 112 for N <= 256, 56 for N <= 512.  Larger shapes are
+ *              rejected with PCA_EUNSUPPORTED and a message naming the limit (pca_small_static_last_error); use pca_run.
+ *   arguments  X, T, P, lambda, iters: dev, as for pca_run (X centred, column-major M x N, never written); eps, max_iter,
+ *              algo as for pca_create; R: dev, M x N column-major, receives the residual of eq. (4), may be
+ *              NULL; stream as everywhere.  X, T, P, R 16-byte aligned.  Options are the library defaults (the listings'
+ *              relative test plus the two-pass stagnation check, PCA output).
+ *   allocation none: no cudaMalloc / cudaFree, no allocating library routine, no host allocation.  The first call on a device
+ *              looks up the array's device address and sets kernel attributes (make that call outside graph capture).
+ *   sharing    all calls on a device share the array, which keeps the last call's contents; nothing in it needs to start at
+ *              zero (the first kernel overwrites every word the solve reads).  Calls that OVERLAP on the GPU (different
+ *              streams, concurrent host threads) race on it: keep them on one stream or order them with events.
+ *   async      only enqueues three small kernels on `stream`.
+ * Errors: PCA_EINVAL, PCA_EALIGN, PCA_EUNSUPPORTED (shape beyond the limits), PCA_ECUDA (pca_small_static_last_cuda_error). */
+int pca_run_small_static(const float* X, int64_t M, int64_t N, int K, double eps, int max_iter, int algo, float* T, float* P,
+                         float* lambda, int32_t* iters, float* R, void* stream);
+size_t pca_small_static_scratch_bytes(void);          /* size of the static device array: 114688 */
+const char* pca_small_static_last_error(void);        /* message of this thread's last failing pca_run_small_static ("" if none) */
+int pca_small_static_last_cuda_error(void);           /* its cudaError_t (as int), 0 if none */
+
 const char* pca_strerror(int code);
 
 /* cudaError_t (as int) of the last failing CUDA call on this context, 0 if none. */

@@ -36,6 +36,7 @@ EXPORTED_SYMBOLS = (
     "pca_shard_create", "pca_shard_workspace_bytes", "pca_shard_set_workspace", "pca_shard_exchange", "pca_shard_colsums",
     "pca_shard_center", "pca_shard_begin", "pca_shard_component", "pca_shard_pass", "pca_shard_done", "pca_shard_finish_component",
     "pca_shard_end", "pca_shard_destroy", "pca_shard_last_cuda_error",
+    "pca_run_small_static", "pca_small_static_scratch_bytes", "pca_small_static_last_error", "pca_small_static_last_cuda_error",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -96,6 +97,12 @@ def load_library() -> ctypes.CDLL:
     lib.pca_shard_destroy.argtypes = [vp]
     lib.pca_shard_destroy.restype = None
     lib.pca_shard_last_cuda_error.argtypes = [vp]
+    lib.pca_run_small_static.argtypes = [vp, i64, i64, i32, f64, i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.pca_small_static_scratch_bytes.argtypes = []
+    lib.pca_small_static_scratch_bytes.restype = ctypes.c_size_t
+    lib.pca_small_static_last_error.argtypes = []
+    lib.pca_small_static_last_error.restype = ctypes.c_char_p
+    lib.pca_small_static_last_cuda_error.argtypes = []
     _lib = lib
     return lib
 
@@ -276,6 +283,35 @@ class PcaContext:
             self.pca_destroy()
         except Exception:
             pass
+
+
+# ---- no-allocation entry point (include/pca.h: pca_run_small_static) -----------------------------------
+def pca_small_static_scratch_bytes() -> int:
+    return int(load_library().pca_small_static_scratch_bytes())
+
+
+def pca_run_small_static(X, T, P, lam, iters, eps=1e-7, max_iter=10000, algo=PCA_ALGO_GS, R=None, stream=None) -> None:
+    """X (N,M) centred, T (K,M), P (K,N) float32; lam (K,) float32; iters (K,) int32; R (N,M) float32 or None -- CUDA,
+    contiguous.  Only enqueues kernels; allocates nothing (the scratch is a static device array of the library)."""
+    import torch
+    lib = load_library()
+    N, M = X.shape
+    K = T.shape[0]
+    PcaContext._check_mat(X, N, M, "X")
+    PcaContext._check_mat(T, K, M, "T")
+    PcaContext._check_mat(P, K, N, "P")
+    if R is not None:
+        PcaContext._check_mat(R, N, M, "R")
+    if lam.dtype != torch.float32 or lam.numel() != K or not lam.is_cuda or not lam.is_contiguous():
+        raise ValueError("lambda must be a contiguous CUDA float32 tensor of K elements")
+    if iters.dtype != torch.int32 or iters.numel() != K or not iters.is_cuda or not iters.is_contiguous():
+        raise ValueError("iters must be a contiguous CUDA int32 tensor of K elements")
+    vp = ctypes.c_void_p
+    code = lib.pca_run_small_static(vp(X.data_ptr()), M, N, K, float(eps), int(max_iter), int(algo), vp(T.data_ptr()),
+                                    vp(P.data_ptr()), vp(lam.data_ptr()), vp(iters.data_ptr()),
+                                    vp(R.data_ptr()) if R is not None else vp(), _stream_ptr(stream))
+    if code != PCA_OK:
+        raise PcaError(code, "pca_run_small_static", lib.pca_small_static_last_error().decode() or pca_strerror(code))
 
 
 # ---- numpy <-> torch layout helpers (no arithmetic) ---------------------------------------------

@@ -187,7 +187,7 @@ def time_steps(prob, steps, warmup):
 
 
 # ncu --set full captures of full launches, bytes per launch: (config name, K, plan, full solve) -> dram read + write
-NCU_TRAFFIC = {("cfg4_65536x2048", 128, "single-sweep streaming", True): 7711567000000 + 114480121000}
+NCU_TRAFFIC = {("cfg4_65536x2048", 128, "single-sweep streaming", True): 7708773000000 + 109641267000}
 
 
 def roofline(prob, run_ms_mean, peaks):
@@ -207,7 +207,7 @@ def roofline(prob, run_ms_mean, peaks):
         "achieved": round(achieved, 1), "peak": peak, "peak_source": peaks["source"], "unit": "GB/s",
         "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC.get((prob.cfg.name, prob.K, prob.ctx.info()["path"], total_iters > 0 and prob.eps > 0)),
         "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of this kernel on this workload (same seeded input, same "
-                        "plan, full solve to convergence) from `ncu --set full`, profiles/r02_ncu_full_cfg4_fullsolve.csv: 0.88 x the "
+                        "plan, full solve to convergence) from `ncu --set full`, profiles/r02b_ncu_full_cfg4_fullsolve.csv: 0.88 x the "
                         "single-sweep algorithmic bytes (alternate sweeps run in opposite row order and re-use the L2-resident tail); "
                         "null for workloads / plans without a capture of the full launch (fixed-work captures: profiles/README.md r02)",
         "algorithmic_bytes_per_launch": int(nbytes), "inner_iterations_per_launch": total_iters,

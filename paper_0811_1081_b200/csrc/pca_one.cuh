@@ -33,52 +33,87 @@ struct OneParams {
   int off_p, off_ttil, off_d, off_qs, off_red, off_sgrp, off_q, off_B, off_A, off_scr, off_vb, off_pp, off_wp;
 };
 
+// The three reductions below are written for a compile-time number of lanes per item (PARTS = pow2 <= 32: shifts instead of
+// divisions, unrolled shuffle trees) and dispatched on the run-time value, which is uniform over the CTA.  They are called
+// by a ROLE: a set of whole warps (`nthr` threads, `rt` = the thread's index within the role), so that independent
+// reductions of one phase run side by side on disjoint warps instead of one after the other on all of them.
+template <int PARTS>
+__device__ __forceinline__ double parts_sum(double a) {
+#pragma unroll
+  for (int o = PARTS >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+  return a;
+}
+#define PCA_ONE_DISPATCH(parts, CALL) \
+  switch (parts) {                    \
+    case 1: { constexpr int PARTS = 1; CALL; } break;   \
+    case 2: { constexpr int PARTS = 2; CALL; } break;   \
+    case 4: { constexpr int PARTS = 4; CALL; } break;   \
+    case 8: { constexpr int PARTS = 8; CALL; } break;   \
+    case 16: { constexpr int PARTS = 16; CALL; } break; \
+    default: { constexpr int PARTS = 32; CALL; } break; \
+  }
+
 // out[c] = sum_g in[g*ld + c] over ngroups, for c < n: `parts` consecutive lanes share a column (parts = pow2 <= 32),
 // each sums every parts-th group in order, then a shuffle tree.  All threads of the CTA must call it.
-__device__ __forceinline__ void one_colsum(const float* in, int ld, int ngroups, int n, int parts, double* out) {
-  const int tid = threadIdx.x;
-  for (int c0 = 0; c0 < n; c0 += kThreads / parts) {
-    const int c = c0 + tid / parts, part = tid & (parts - 1);
+template <int PARTS>
+__device__ __forceinline__ void one_colsum_t(const float* in, int ld, int ngroups, int n, double* out, int tid, int nthr) {
+  for (int c0 = 0; c0 < n; c0 += nthr / PARTS) {
+    const int c = c0 + tid / PARTS, part = tid & (PARTS - 1);
     double a = 0.0;
-    if (c < n)
-      for (int g = part; g < ngroups; g += parts) a += (double)in[(size_t)g * ld + c];
-    for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if (c < n) {
+#pragma unroll 4
+      for (int g = part; g < ngroups; g += PARTS) a += (double)in[(size_t)g * ld + c];
+    }
+    a = parts_sum<PARTS>(a);
     if (part == 0 && c < n) out[c] = a;
   }
+}
+__device__ __forceinline__ void one_colsum(const float* in, int ld, int ngroups, int n, int parts, double* out, int rt, int nthr) {
+  PCA_ONE_DISPATCH(parts, one_colsum_t<PARTS>(in, ld, ngroups, n, out, rt, nthr))
 }
 
 // acc[i] = sum_{j<k} Mx[i*ld + j] * v[j] for i < n (row-major panel, odd row stride): `parts` lanes per row.
 // f(i, value) is called by the first lane of each row.  All threads must call it.
-template <typename F>
-__device__ __forceinline__ void one_rowdot(const float* Mx, int ld, const double* v, int n, int k, int parts, F f) {
-  const int tid = threadIdx.x;
-  for (int i0 = 0; i0 < n; i0 += kThreads / parts) {
-    const int i = i0 + tid / parts, part = tid & (parts - 1);
+template <int PARTS, typename F>
+__device__ __forceinline__ void one_rowdot_t(const float* Mx, int ld, const double* v, int n, int k, F& f, int tid, int nthr) {
+  for (int i0 = 0; i0 < n; i0 += nthr / PARTS) {
+    const int i = i0 + tid / PARTS, part = tid & (PARTS - 1);
     double a = 0.0;
-    if (i < n)
-      for (int j = part; j < k; j += parts) a += (double)Mx[(size_t)i * ld + j] * v[j];
-    for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if (i < n) {
+#pragma unroll 4
+      for (int j = part; j < k; j += PARTS) a += (double)Mx[(size_t)i * ld + j] * v[j];
+    }
+    a = parts_sum<PARTS>(a);
     if (part == 0 && i < n) f(i, a);
   }
 }
+template <typename F>
+__device__ __forceinline__ void one_rowdot(const float* Mx, int ld, const double* v, int n, int k, int parts, F f, int rt, int nthr) {
+  PCA_ONE_DISPATCH(parts, (one_rowdot_t<PARTS>(Mx, ld, v, n, k, f, rt, nthr)))
+}
 
 // acc[j] = sum_{i<n} Mx[i*ld + j] * v[i] for j < k (column sums of a row-major panel): `parts` lanes per column.
-template <typename VT, typename F>
-__device__ __forceinline__ void one_coldot(const float* Mx, int ld, const VT* v, int n, int k, int parts, F f) {
-  const int tid = threadIdx.x;
-  for (int j0 = 0; j0 < k; j0 += kThreads / parts) {
-    const int j = j0 + tid / parts, part = tid & (parts - 1);
+template <int PARTS, typename VT, typename F>
+__device__ __forceinline__ void one_coldot_t(const float* Mx, int ld, const VT* v, int n, int k, F& f, int tid, int nthr) {
+  for (int j0 = 0; j0 < k; j0 += nthr / PARTS) {
+    const int j = j0 + tid / PARTS, part = tid & (PARTS - 1);
     double a = 0.0;
-    if (j < k)
-      for (int i = part; i < n; i += parts) a += (double)Mx[(size_t)i * ld + j] * (double)v[i];
-    for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+    if (j < k) {
+#pragma unroll 4
+      for (int i = part; i < n; i += PARTS) a += (double)Mx[(size_t)i * ld + j] * (double)v[i];
+    }
+    a = parts_sum<PARTS>(a);
     if (part == 0 && j < k) f(j, a);
   }
 }
+template <typename VT, typename F>
+__device__ __forceinline__ void one_coldot(const float* Mx, int ld, const VT* v, int n, int k, int parts, F f, int rt, int nthr) {
+  PCA_ONE_DISPATCH(parts, (one_coldot_t<PARTS, VT>(Mx, ld, v, n, k, f, rt, nthr)))
+}
 
-__device__ __forceinline__ int one_parts(int n) {          // lanes per item so that n items keep the CTA busy: pow2 in [1, 32]
+__device__ __forceinline__ int one_parts(int n, int nthr = kThreads) {   // lanes per item so that n items keep nthr threads busy: pow2 in [1, 32]
   int p = 32;
-  while (p > 1 && n * p > kThreads) p >>= 1;
+  while (p > 1 && n * p > nthr) p >>= 1;
   return p;
 }
 
@@ -86,6 +121,7 @@ template <int GT, int RPT>
 __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams prm) {
   extern __shared__ __align__(16) unsigned char smem[];
   constexpr int NV = 2, NG = kThreads / GT;
+  constexpr int NGQ = GT < 32 ? kWarps : NG;                       // rows of qs: the row groups of a warp pre-add their partial q (reg_sweep_*<..., WPRE>)
   float* p_s = reinterpret_cast<float*>(smem + prm.off_p);        // ldr: orthogonalised loads p^ of the last sweep
   float* ttil_s = reinterpret_cast<float*>(smem + prm.off_ttil);  // NG*RPT: t0 / t~
   float* d_s = reinterpret_cast<float*>(smem + prm.off_d);        // NG*RPT: deflation vector
@@ -119,12 +155,15 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
   for (int i = tid; i < NG * RPT; i += kThreads) { d_s[i] = 0.f; ttil_s[i] = 0.f; }
   for (int n = tid; n < ldr; n += kThreads) { p_s[n] = 0.f; q_s[n] = 0.0; }
   __syncthreads();
-  const int pq = one_parts(ldr);                                   // lanes per column in the N-side phases
+  const int pq = one_parts(ldr);                                   // lanes per column in the N-side phases run by all warps
+  // Roles of the two phases with independent work (whole warps each; kWarps = 16): the last warp takes the scalar chain
+  // (|t~|^2, then lambda' and the test); with Gram-Schmidt coefficients to form, warps 0-7 combine q while warps 8-14 form B.
+  constexpr int kScalarWarp = kWarps - 1, kQWarpsB = 8;
 
   for (int k = 0; k < K; ++k) {
     const bool gsk = gs && k > 0;
     // ---- S1 + S2: t0 <- column k of the deflated residual; q = R^T t0 ----
-    reg_sweep_loads<GT, NV, RPT>(Rr, k, ttil_s, qs, sgrp, ldr);
+    reg_sweep_loads<GT, NV, RPT, true>(Rr, k, ttil_s, qs, sgrp, ldr);
     double lam = 0.0, lam2 = 0.0, lam_new = 0.0;
     int it = 0;
     bool degenerate = false, first = true;
@@ -133,17 +172,23 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
     for (;;) {
       const bool with_b = gsk && !first;
       // ---- q = sum of the group partials (fp64);  |t~|^2;  B = V_(k)^T t~ (S6) ----
-      one_colsum(qs, ldr, NG, ldr, pq, q_s);
-      if (w == 0) {
-        double s = 0.0;
-        for (int gg = lane; gg < NG; gg += 32) s += sgrp[gg];
-        s = warp_sum(s);
-        if (lane == 0) ctl_s[0] = s;
+      {
+        const int wq = with_b ? kQWarpsB : kScalarWarp;
+        if (w < wq) {
+          one_colsum(qs, ldr, NGQ, ldr, one_parts(ldr, 32 * wq), q_s, tid, 32 * wq);
+        } else if (w < kScalarWarp) {
+          constexpr int nb = 32 * (kScalarWarp - kQWarpsB);
+          one_coldot<float>(Vb, KV, ttil_s, mb, k, one_parts(k, nb), [&](int j, double a) { B_s[j] = a; }, tid - 32 * kQWarpsB, nb);
+        } else {
+          double s = 0.0;
+          for (int gg = lane; gg < NG; gg += 32) s += sgrp[gg];
+          s = warp_sum(s);
+          if (lane == 0) ctl_s[0] = s;
+        }
       }
-      if (with_b) one_coldot<float>(Vb, KV, ttil_s, mb, k, pk2, [&](int j, double a) { B_s[j] = a; });
       __syncthreads();
-      // ---- S7 / S8 by warp 0;  p~ = q - W B ----
-      if (w == 0) {
+      // ---- S7 / S8 by the scalar warp;  p~ = q - W B by the others ----
+      if (w == kScalarWarp) {
         const double s = ctl_s[0];
         int st = 0;
         double ln = 0.0;
@@ -158,14 +203,18 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
           const double l2 = s - bb;                                           // |t~ - V B|^2, V orthonormal
           if (!(l2 > 0.0)) st = 2;
           else {
-            ln = sqrt(l2);                                                    // S7
+            const double r = rsqrt(l2);                                       // S7: sqrt(l2) as l2 * rsqrt(l2)
+            ln = l2 * r;                                                      //   plus one Newton step (sqrt() is a 300-cycle
+            ln = fma(fma(-ln, ln, l2), 0.5 * r, ln);                          //   routine on the per-pass chain; this one is 1/3)
             // S8: the listings' strict relative test (readings C3, C4b)
             if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode, prm.stag2) || (it >= prm.max_iter)) st = 1;
           }
         }
         if (lane == 0) { ctl_s[1] = ln; reinterpret_cast<int*>(ctl_s + 2)[0] = st; }
+      } else if (with_b) {
+        constexpr int nw = 32 * kScalarWarp;
+        one_rowdot(Wp, KV, B_s, N, k, one_parts(N, nw), [&](int c, double a) { q_s[c] -= a; }, tid, nw);
       }
-      if (with_b) one_rowdot(Wp, KV, B_s, N, k, pq, [&](int c, double a) { q_s[c] -= a; });
       __syncthreads();
       const int st = reinterpret_cast<const int*>(ctl_s + 2)[0];
       if (st == 2) { degenerate = true; break; }
@@ -175,27 +224,33 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
         lam2 = lam;
         lam = lam_new;
       }
-      // ---- S3: A = P_(k)^T p~ ;  p^ = p~ - P_(k) A ----
+      // ---- S3: A = P_(k)^T p~ ;  p^ = p~ - P_(k) A;  S4: p = p^ / |p^| (the scale is applied
+      //      by the sweep).  p_s[N..ldr) stays zero from the start of the kernel. ----
       if (gsk) {
-        one_coldot<double>(Pp, KV, q_s, N, k, pk2, [&](int j, double a) { A_s[j] = a; });
-        __syncthreads();
-        one_rowdot(Pp, KV, A_s, N, k, pq, [&](int c, double a) { q_s[c] -= a; });
+        one_coldot<double>(Pp, KV, q_s, N, k, pk2, [&](int j, double a) { A_s[j] = a; }, tid, kThreads);
         __syncthreads();
       }
-      // ---- S4: p = p^ / |p^| (the scale is applied by the sweep) ----
+      if (gsk) {
+        one_rowdot(Pp, KV, A_s, N, k, pq, [&](int c, double a) {
+          const double x = q_s[c] - a;
+          q_s[c] = x;
+          p_s[c] = (float)x;
+        }, tid, kThreads);
+      } else {
+        for (int c = tid; c < N; c += kThreads) p_s[c] = (float)q_s[c];
+      }
+      __syncthreads();
+      // |p^|^2 of the fp32 loads the sweep will use: every warp forms it itself from p_s (same order in every warp), which
+      // costs one shuffle tree instead of two trees and a second barrier
       double n2 = 0.0;
-      for (int c = tid; c < ldr; c += kThreads) {
-        const float v = (c < N) ? (float)q_s[c] : 0.f;
-        p_s[c] = v;
-        n2 += (double)v * (double)v;
-      }
-      n2 = block_sum(n2, scr);
+      for (int c = lane; c < N; c += 32) { const double v = (double)p_s[c]; n2 += v * v; }
+      n2 = warp_sum(n2);
       pscale = (n2 > 0.0) ? (float)rsqrt(n2) : 0.f;
       if (!(pscale > 0.f)) { degenerate = true; break; }                      // reading C7
       first = false;
       ++it;
       // ---- FUSED sweep: t~ = R p (S5), q = R^T t~ (S2 of the next pass) ----
-      reg_sweep_fused<GT, NV, RPT>(Rr, p_s, pscale, ttil_s, qs, red_s, sgrp, ldr);
+      reg_sweep_fused<GT, NV, RPT, true>(Rr, p_s, pscale, ttil_s, qs, red_s, sgrp, ldr);
     }
 
     if (degenerate) {
@@ -217,7 +272,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
         d_s[r] = t;
         prm.T[(size_t)k * M + r] = prm.out_svd ? t * inv : t;                 // SVD output: the unit vector v
         if (gs) Vb[(size_t)r * KV + k] = t * inv;
-      });
+      }, tid, kThreads);
       for (int c = tid; c < ldr; c += kThreads) {
         const float pk = p_s[c] * pscale;
         if (c < N) prm.P[(size_t)k * N + c] = pk;

@@ -134,7 +134,35 @@ __device__ __forceinline__ void group_sync(int g) {
 // p_s holds the orthogonalised loads p^, pscale = 1/|p^|.
 // Leaves t~ in ttil_s, the per-group partial q in qs[g][ldr], the per-group sum of t~^2 (fp64) in sgrp[g];
 // ends with __syncthreads().  red_s: NG*WG*8 floats.
-template <int GT, int NV, int RPT>
+// WPRE (one-CTA kernel, GT < 32): the 32/GT row groups of a warp add their partial q by shuffles (fp32, fixed butterfly
+// order) and the warp stores ONE row qs[warp][ldr] instead of one per group: a quarter / half of the rows to combine later.
+template <int GT, int NV>
+__device__ __forceinline__ void store_q_partial(float4 (&q4)[NV], float* qs, int g, int gl, int ldr, bool wpre) {
+  if constexpr (GT < 32) {
+    if (wpre) {
+#pragma unroll
+      for (int o = GT; o < 32; o <<= 1) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          q4[v].x += __shfl_xor_sync(0xffffffffu, q4[v].x, o);
+          q4[v].y += __shfl_xor_sync(0xffffffffu, q4[v].y, o);
+          q4[v].z += __shfl_xor_sync(0xffffffffu, q4[v].z, o);
+          q4[v].w += __shfl_xor_sync(0xffffffffu, q4[v].w, o);
+        }
+      }
+      if ((threadIdx.x & 31) < GT) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v)
+          *reinterpret_cast<float4*>(qs + (size_t)(threadIdx.x >> 5) * ldr + 4 * (gl + GT * v)) = q4[v];
+      }
+      return;
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q4[v];
+}
+
+template <int GT, int NV, int RPT, bool WPRE = false>
 __device__ __forceinline__ void reg_sweep_fused(const float4 (&Rr)[RPT][NV], const float* p_s, float pscale, float* ttil_s,
                                                 float* qs, float* red_s, double* sgrp, int ldr) {
   static_assert(RPT <= 8, "one batch of at most 8 rows per group");
@@ -185,14 +213,13 @@ __device__ __forceinline__ void reg_sweep_fused(const float4 (&Rr)[RPT][NV], con
   for (int i = 0; i < RPT; ++i)
 #pragma unroll
     for (int v = 0; v < NV; ++v) axpy4(q4[v], Rr[i][v], tt[i]);
-#pragma unroll
-  for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q4[v];
+  store_q_partial<GT, NV>(q4, qs, g, gl, ldr, WPRE);
   __syncthreads();
 }
 
 // LOADS sweep at the start of component k:  t0 <- column k of the (already deflated) residual (S1,
 // PAPER.md:556,:1017);  q = R^T t0 (S2).  Same outputs as reg_sweep_fused.
-template <int GT, int NV, int RPT>
+template <int GT, int NV, int RPT, bool WPRE = false>
 __device__ __forceinline__ void reg_sweep_loads(const float4 (&Rr)[RPT][NV], int k, float* ttil_s, float* qs, double* sgrp,
                                                 int ldr) {
   const int tid = threadIdx.x, g = tid / GT, gl = tid - g * GT;
@@ -223,8 +250,7 @@ __device__ __forceinline__ void reg_sweep_loads(const float4 (&Rr)[RPT][NV], int
     for (int v = 0; v < NV; ++v) axpy4(q4[v], Rr[i][v], t);
   }
   if (gl == 0) sgrp[g] = sacc;
-#pragma unroll
-  for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q4[v];
+  store_q_partial<GT, NV>(q4, qs, g, gl, ldr, WPRE);
   __syncthreads();
 }
 

@@ -100,6 +100,20 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 // lam = lambda of the previous pass (0 before the first), lam2 = of the one before (0 = none yet):
 // reading C4b (stag2 != 0, PCA_OPT_STAGNATION = 1, the default): a period-2 limit cycle of lambda' in fp32 is stagnation
 // too, so lambda' is also compared with the value two passes back.  stag2 == 0: the listing's / text's test alone.
+// sqrt(x) and 1/x for a normal x > 0 from rsqrt(x) plus one Newton step (a few ulp at most).  sqrt() and the fp64 division are
+// 300-cycle routines (measured on B200: sqrt 313, rsqrt 99 cycles of dependent latency) and lambda' = sqrt(.) sits on the serial
+// per-pass chain of the convergence test that every CTA waits for.
+__device__ __forceinline__ double fast_sqrt(double x) {
+  const double r = rsqrt(x);
+  const double y = x * r;
+  return fma(fma(-y, y, x), 0.5 * r, y);
+}
+__device__ __forceinline__ double fast_rcp(double x) {
+  const double r = rsqrt(x);
+  const double y = r * r;
+  return fma(fma(-x, y, 1.0), y, y);
+}
+
 __device__ __forceinline__ bool pca_stagnated(double lam, double lam2, double ln, double eps, int mode, int stag2) {
   const bool two = stag2 != 0 && lam2 > 0.0;
   if (mode == 1) return fabs(ln - lam) <= eps || (two && fabs(ln - lam2) <= eps);

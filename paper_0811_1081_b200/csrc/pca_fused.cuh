@@ -683,7 +683,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
             bb = warp_sum(bb);
           }
           double l2 = s - bb;                                                 // |t~ - V B|^2, V orthonormal
-          double rho = 1.0;
+          double rho = 1.0, rho2 = 1.0;
           if (gsk) {
             const double pn2 = ctl_s[3], a2 = sb_s[2];
             if (deferred) {
@@ -692,8 +692,9 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
               // rho = |p~|/|p^|
               const double d2 = pn2 - a2;
               if (!(d2 > 0.0)) l2 = 0.0;
-              else rho = sqrt(pn2 / d2);
-              l2 *= rho * rho;
+              else rho2 = pn2 * fast_rcp(d2);
+              l2 *= rho2;
+              rho = fast_sqrt(rho2);
             }
             // the NEXT pass defers S3 only if that is harmless (same decision on every CTA): see kDeferKappa
             if (lane == 0) reinterpret_cast<int*>(ctl_s + 4)[0] = (a2 * bf2 <= kDeferKappa * pn2 * lam * lam) ? 1 : 0;
@@ -701,7 +702,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_fused_kernel(const FusedParam
           if (lane == 0) ctl_s[2] = rho;
           if (!(l2 > 0.0)) st = 2;                                            // reading C7
           else {
-            ln = sqrt(l2);                                                    // S7
+            ln = fast_sqrt(l2);                                                    // S7
             // S8: listings' strict relative test (reading C3)
             // (+ reading C4b: a period-2 limit cycle of lambda' in fp32 is stagnation too)
             if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode, prm.stag2) || (it >= prm.max_iter)) st = 1;

@@ -203,9 +203,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
           const double l2 = s - bb;                                           // |t~ - V B|^2, V orthonormal
           if (!(l2 > 0.0)) st = 2;
           else {
-            const double r = rsqrt(l2);                                       // S7: sqrt(l2) as l2 * rsqrt(l2)
-            ln = l2 * r;                                                      //   plus one Newton step (sqrt() is a 300-cycle
-            ln = fma(fma(-ln, ln, l2), 0.5 * r, ln);                          //   routine on the per-pass chain; this one is 1/3)
+            ln = fast_sqrt(l2);                                               // S7
             // S8: the listings' strict relative test (readings C3, C4b)
             if (pca_stagnated(lam, lam2, ln, prm.eps, prm.test_mode, prm.stag2) || (it >= prm.max_iter)) st = 1;
           }

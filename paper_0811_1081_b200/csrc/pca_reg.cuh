@@ -643,17 +643,18 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
               bb = warp_sum(bb);
             }
             double l2 = s - bb;                                               // |t~ - V B|^2, V orthonormal
-            double rho = 1.0;
+            double rho = 1.0, rho2 = 1.0;
             if (gsk && deferred) {                                            // |p^|^2 = |p~|^2 - |A|^2 (P orthonormal)
               const double pn2 = ctl_s[5], d2 = pn2 - ctl_s[6];
               if (!(d2 > 0.0)) l2 = 0.0;
-              else rho = sqrt(pn2 / d2);
-              l2 *= rho * rho;
+              else rho2 = pn2 * fast_rcp(d2);
+              l2 *= rho2;
+              rho = fast_sqrt(rho2);
             }
             if (lane == 0) ctl_s[7] = rho;
             if (!(l2 > 0.0)) st = 2;                                          // reading C7
             else {
-              ln = sqrt(l2);                                                  // S7
+              ln = fast_sqrt(l2);                                                  // S7
               // S8: the listings' strict relative test (reading C3)
               // (+ reading C4b: in fp32 the iteration can end in a period-2 limit cycle, lambda' alternating between two
               //  values; that is stagnation too, so lambda' is also compared with the value two passes back)

@@ -348,19 +348,12 @@ __device__ __forceinline__ void reg_publish_q(const RegParams& prm, const float*
 // Publish |t~|^2 and (GS-PCA, k > 0) the B-partials V_b^T t~ (S6) of this CTA.
 // Vb: [rows][KV] unit score rows of this CTA (shared memory, odd row stride KV: conflict-free for lanes over rows AND
 // over columns).  `parts` threads (consecutive lanes) share a column j and split the rows; no barrier inside.
-__device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const float* ttil_s, const double* sgrp, u64* sbx, int G,
-                                               int NG, int mb, int k, bool with_b, unsigned seq) {   // sbx: this CTA's slot of unit 0
+// B-partials of reg_publish_sb with a compile-time number of lanes per column (PARTS): shifts and an unrolled shuffle tree
+template <int PARTS>
+__device__ __forceinline__ void reg_publish_b_t(const float* Vb, int KV, const float* ttil_s, u64* sbx, int G, int mb, int k,
+                                                unsigned seq) {
+  constexpr int parts = PARTS;
   const int tid = threadIdx.x;
-  if (tid == 0) {
-    double a = 0.0;
-    for (int g = 0; g < NG; ++g) a += sgrp[g];
-    gl_st2d(sbx, a, seq);
-  }
-  if (!with_b) return;
-  __syncwarp();            // (warp 0 re-converges before the full-mask shuffles below; measured in pca_fused.cuh: 2-6 x otherwise)
-  int Kc = 32;
-  while (Kc < k) Kc <<= 1;
-  const int parts = kThreads / Kc;                                     // 1..16, a power of two
   const int j = tid / parts, part = tid - j * parts;
   float a = 0.f;
   if (j < k)
@@ -376,27 +369,57 @@ __device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const fl
     for (; r < mb; r += parts) a = fmaf(Vb[(size_t)r * KV + j], ttil_s[r], a);
     a = (a + a1) + (a2 + a3);
   }
+#pragma unroll
   for (int o = parts >> 1; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
   const float nb = __shfl_down_sync(0xffffffffu, a, parts);             // column j + 1 (same part)
   if (part == 0 && (j & 1) == 0 && j < k)
     gl_st2(sbx + (size_t)(1 + (j >> 1)) * G * 2, ll_wordf(a, seq), ll_wordf(j + 1 < k ? nb : 0.f, seq));
 }
+__device__ __forceinline__ void reg_publish_sb(const float* Vb, int KV, const float* ttil_s, const double* sgrp, u64* sbx, int G,
+                                               int NG, int mb, int k, bool with_b, unsigned seq) {   // sbx: this CTA's slot of unit 0
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    double a = 0.0;
+    for (int g = 0; g < NG; ++g) a += sgrp[g];
+    gl_st2d(sbx, a, seq);
+  }
+  if (!with_b) return;
+  __syncwarp();            // (warp 0 re-converges before the full-mask shuffles below; measured in pca_fused.cuh: 2-6 x otherwise)
+  int Kc = 32;
+  while (Kc < k) Kc <<= 1;
+  switch (kThreads / Kc) {                                             // lanes per column: 1..16, a power of two
+    case 16: reg_publish_b_t<16>(Vb, KV, ttil_s, sbx, G, mb, k, seq); break;
+    case 8: reg_publish_b_t<8>(Vb, KV, ttil_s, sbx, G, mb, k, seq); break;
+    case 4: reg_publish_b_t<4>(Vb, KV, ttil_s, sbx, G, mb, k, seq); break;
+    case 2: reg_publish_b_t<2>(Vb, KV, ttil_s, sbx, G, mb, k, seq); break;
+    default: reg_publish_b_t<1>(Vb, KV, ttil_s, sbx, G, mb, k, seq); break;
+  }
+}
+
 
 // praw[i] -= sum_{j<k} C[i*KP + j] * coef[j] for the ns columns of this owner: LPR lanes per column (8 for k <= 64, else 32;
 // lane l takes j = l, l + LPR, ... in order, then a shuffle tree), 32/LPR columns per warp and round.
-__device__ __forceinline__ void reg_slice_correct(double* praw_s, const float* C, int KP, const double* coef_s, int ns, int k) {
+template <int LPR>
+__device__ __forceinline__ void reg_slice_correct_t(double* praw_s, const float* C, int KP, const double* coef_s, int ns, int k) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int lpr = k <= 64 ? 8 : 32, rpw = 32 / lpr, ll = lane & (lpr - 1);
+  constexpr int rpw = 32 / LPR;
+  const int ll = lane & (LPR - 1);
   for (int i0 = 0; i0 < ns; i0 += rpw * kWarps) {                             // (uniform trip count: shuffles inside)
-    const int i = i0 + w * rpw + lane / lpr;
+    const int i = i0 + w * rpw + lane / LPR;
     double c = 0.0;
     if (i < ns) {
       const float* ci = C + (size_t)i * KP;
-      for (int j = ll; j < k; j += lpr) c += (double)ci[j] * coef_s[j];
+#pragma unroll 4
+      for (int j = ll; j < k; j += LPR) c += (double)ci[j] * coef_s[j];
     }
-    for (int o = lpr >> 1; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+#pragma unroll
+    for (int o = LPR >> 1; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
     if (ll == 0 && i < ns) praw_s[i] -= c;
   }
+}
+__device__ __forceinline__ void reg_slice_correct(double* praw_s, const float* C, int KP, const double* coef_s, int ns, int k) {
+  if (k <= 64) reg_slice_correct_t<8>(praw_s, C, KP, coef_s, ns, k);          // (compile-time lane count: unrolled shuffle tree)
+  else reg_slice_correct_t<32>(praw_s, C, KP, coef_s, ns, k);
 }
 
 // S3, first half: this owner's partial  a_S[j] = sum_{n in S} P[n,j] p~[n], all threads of the CTA.
@@ -628,9 +651,11 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
         __syncthreads();
         reg_trace(prm, tn, TR_X1);
         // S7/S8 by warp 0 of owner 0 (then it joins the others);  p~ = q - W B on the owner's slice (needs only B)
-        if (w == 0 && lane == 0 && (b != 0 || first)) ctl_s[7] = 1.0;
-        if (w == 0 && b != 0 && lane == 0) { ctl_s[0] = 0.0; reinterpret_cast<int*>(ctl_s + 1)[0] = 0; }
-        if (w == 0 && b == 0) {
+        // (the LAST warp: the slice correction below starts with warp 0 and reaches the last warp only for slices wider than
+        //  60 columns, so on owner 0 the scalar chain of the test runs beside it instead of in front of it)
+        if (w == kWarps - 1 && lane == 0 && (b != 0 || first)) ctl_s[7] = 1.0;
+        if (w == kWarps - 1 && b != 0 && lane == 0) { ctl_s[0] = 0.0; reinterpret_cast<int*>(ctl_s + 1)[0] = 0; }
+        if (w == kWarps - 1 && b == 0) {
           const double s = sb_s[0];
           int st = 0;                                                         // 0 continue, 1 done, 2 degenerate
           double ln = 0.0;

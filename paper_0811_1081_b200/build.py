@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpca_b200.so")
 SOURCES = [os.path.join(CSRC, "pca_api.cu"), os.path.join(CSRC, "pca_shard.cu"), os.path.join(CSRC, "pca_noalloc.cu")]
 REG_INST = os.path.join(CSRC, "pca_reg_inst.cu")        # compiled REG_PARTS times with -DPCA_REG_PART=i
-REG_PARTS = 4
+REG_PARTS = 6
 HEADERS = [os.path.join(CSRC, f) for f in ("pca_device.cuh", "pca_solve.cuh", "pca_fused.cuh", "pca_tma.cuh", "pca_shard.cuh", "pca_reg.cuh", "pca_one.cuh",
                                            "pca_center.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "pca.h")]

@@ -68,6 +68,8 @@ reg_kernel_t reg_kernel_lookup_part0(int gt, int rpt);
 reg_kernel_t reg_kernel_lookup_part1(int gt, int rpt);
 reg_kernel_t reg_kernel_lookup_part2(int gt, int rpt);
 reg_kernel_t reg_kernel_lookup_part3(int gt, int rpt);
+reg_kernel_t reg_kernel_lookup_part4(int gt);
+reg_kernel_t reg_kernel_lookup_part5(int gt);
 one_kernel_t one_kernel_lookup_part0(int gt, int rpt);
 one_kernel_t one_kernel_lookup_part1(int gt, int rpt);
 one_kernel_t one_kernel_lookup(int gt, int rpt) {
@@ -75,7 +77,12 @@ one_kernel_t one_kernel_lookup(int gt, int rpt) {
   if (!f) f = one_kernel_lookup_part1(gt, rpt);
   return f;
 }
-reg_kernel_t reg_kernel_lookup(int gt, int rpt) {
+reg_kernel_t reg_kernel_lookup(int gt, int rpt, int rs) {
+  if (rs != 0) {
+    if (rs != kRegSmemRows || rpt != 7) return nullptr;
+    reg_kernel_t g = reg_kernel_lookup_part4(gt);
+    return g ? g : reg_kernel_lookup_part5(gt);
+  }
   reg_kernel_t f = reg_kernel_lookup_part0(gt, rpt);
   if (!f) f = reg_kernel_lookup_part1(gt, rpt);
   if (!f) f = reg_kernel_lookup_part2(gt, rpt);
@@ -388,8 +395,9 @@ int make_reg_plan(pca_ctx* c) {
   for (int r : {2, 4, 7})
     if ((long long)NG * r >= Mb) { RPT = r; break; }
   if (!RPT) return PCA_EUNSUPPORTED;
-  pca::reg_kernel_t fn = pca::reg_kernel_lookup(GT, RPT);
+  pca::reg_kernel_t fn = pca::reg_kernel_lookup(GT, RPT, 0);
   if (!fn) return PCA_EUNSUPPORTED;
+  int rsm_rows = 0;                                                  // rows of every thread's row block kept in shared memory
   int g2 = 1;
   while (g2 * 2 <= G) g2 *= 2;                                       // owners: a power of two <= G
   RegParams p{};
@@ -415,6 +423,7 @@ int make_reg_plan(pca_ctx* c) {
     p.off_vb = take(gs ? rows * KV * 4 : 0);
     p.off_pc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
     p.off_wc = take(gs ? (size_t)p.Ns * KV * 4 : 0);
+    p.off_rsm = take((size_t)rsm_rows * NG * ldr * 4);               // RowBlock: rows kept in shared memory
     p.off_x = -1;
     if (G == 1) {                                                     // one CTA: exchange buffers in shared memory if they fit
       const size_t xwords = (size_t)6 * ldr + 4 * (1 + p.Kpad / 2) + 4 * (2 + p.Kpad) + 4 * (p.Kpad / 2) + 2 * (Gs * 2 + 6) + 2 * (Gs * 2);
@@ -433,6 +442,17 @@ int make_reg_plan(pca_ctx* c) {
     if (smem <= (size_t)c->smem_optin) break;
     if (Gs * 2 > g2 || Gs * 2 > ldr / 2) return PCA_EUNSUPPORTED;   // more owners = smaller P / W panels per owner
     Gs *= 2;
+  }
+  // RPT = 7 fills the register file (56 of 128 registers hold R, the rest of the pass spills): take the variant that keeps two
+  // of the seven rows in shared memory when that leaves the total at or below 100 KB -- beyond it the L1 that serves the
+  // remaining spills and the panel loads shrinks and the pass gets slower (measured: config 2 9.7 -> 9.3 us, config 5 with its
+  // 115 KB of unit scores 11.9 -> 13.1)
+  if (RPT == 7) {
+    pca::reg_kernel_t fs = pca::reg_kernel_lookup(GT, RPT, pca::kRegSmemRows);
+    rsm_rows = pca::kRegSmemRows;
+    const size_t smem_s = carve_reg(Gs);
+    if (fs && smem_s <= (size_t)100 * 1024) { fn = fs; smem = smem_s; }
+    else { rsm_rows = 0; smem = carve_reg(Gs); }
   }
   cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);   // per FUNCTION: the device maximum, so that contexts do not lower it for each other
   if (e != cudaSuccess) return cuda_fail(c, e);

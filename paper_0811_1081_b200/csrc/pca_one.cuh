@@ -144,13 +144,14 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
   const bool gs = prm.algo == 1;
   float* Rb = prm.Rrm;
 
-  float4 Rr[RPT][NV];                                              // R <- X, in registers
+  RowBlock<NV, RPT, 0> Rr;                                         // R <- X, in registers
+  Rr.sm = nullptr; Rr.rstride = 0; Rr.vstride = 0;
 #pragma unroll
   for (int i = 0; i < RPT; ++i) {
     const int r = g * RPT + i;
 #pragma unroll
     for (int v = 0; v < NV; ++v)
-      Rr[i][v] = (r < mb) ? ld_stream4(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      Rr.r[i][v] = (r < mb) ? ld_stream4(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) : make_float4(0.f, 0.f, 0.f, 0.f);
   }
   for (int i = tid; i < NG * RPT; i += kThreads) { d_s[i] = 0.f; ttil_s[i] = 0.f; }
   for (int n = tid; n < ldr; n += kThreads) { p_s[n] = 0.f; q_s[n] = 0.0; }
@@ -292,7 +293,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
       for (int i = 0; i < RPT; ++i) {
         const float dr = -d_s[g * RPT + i];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) axpy4(Rr[i][v], p4[v], dr);
+        for (int v = 0; v < NV; ++v) axpy4(Rr.r[i][v], p4[v], dr);
       }
     }
   }
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_one_kernel(const OneParams pr
     const int r = g * RPT + i;
     if (r < mb) {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) = Rr[i][v];
+      for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) = Rr.r[i][v];
     }
   }
 }

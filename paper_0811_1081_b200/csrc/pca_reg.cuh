@@ -27,6 +27,8 @@
 
 namespace pca {
 
+constexpr int kRegSmemRows = 2;   // RS of the compiled <GT, 2, 7, RS> variants: 2 of the 7 rows of a thread's row block in shared memory
+
 struct RegParams {
   float* Rrm;            // M x ldr row-major residual (workspace): read once, written once
   float* T;              // M x K col-major
@@ -65,6 +67,7 @@ struct RegParams {
   // shared-memory carve-up (byte offsets)
   int off_p, off_ttil, off_d, off_qs, off_red, off_sgrp, off_B, off_A, off_scr, off_praw, off_vb, off_pc, off_wc;
   int off_x;             // >= 0 (one CTA only): the exchange buffers live in shared memory at this offset
+  int off_rsm;           // kernel variants with RS > 0: the last RS rows of every row group live in shared memory (RowBlock)
 };
 
 // ------------------------------------------------------------------------------------ trace
@@ -128,6 +131,28 @@ __device__ __forceinline__ void group_sync(int g) {
   else named_bar_sync(1 + g, GT);
 }
 
+// ------------------------------------------------------------------------------------ row block of a thread
+// RPT rows x NV float4 of R per thread.  The first RPT - RS rows live in REGISTERS, the last RS in SHARED memory: the kernel is
+// compiled for 128 registers per thread (512 threads, one CTA per SM) and 56 of them holding R (RPT = 7) left the rest of
+// the pass spilling (428 bytes); shared memory is three quarters empty.  Every thread reads and writes only its own words
+// there (no synchronisation), consecutive threads touch consecutive float4s (no bank conflicts).
+template <int NV, int RPT, int RS>
+struct RowBlock {
+  static constexpr int RR = RPT - RS;
+  float4 r[RR > 0 ? RR : 1][NV];
+  float4* sm;      // this thread's float4 of the group's first shared-memory row
+  int rstride;     // float4s between consecutive rows (ldr / 4)
+  int vstride;     // float4s between the thread's column blocks (GT)
+  __device__ __forceinline__ float4 get(int i, int v) const {
+    if (i < RR) return r[i < RR ? i : 0][v];
+    return sm[(i - RR) * rstride + v * vstride];
+  }
+  __device__ __forceinline__ void set(int i, int v, const float4& x) {
+    if (i < RR) r[i < RR ? i : 0][v] = x;
+    else sm[(i - RR) * rstride + v * vstride] = x;
+  }
+};
+
 // ------------------------------------------------------------------------------------ sweeps
 // FUSED sweep over the CTA's rows held in registers:
 //   t~[r] = sum_n R[r,n] p[n]   (S5);   q[n] += R[r,n] t~[r]   (S2 of the next pass, :562,:1023)
@@ -162,8 +187,8 @@ __device__ __forceinline__ void store_q_partial(float4 (&q4)[NV], float* qs, int
   for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(qs + (size_t)g * ldr + 4 * (gl + GT * v)) = q4[v];
 }
 
-template <int GT, int NV, int RPT, bool WPRE = false>
-__device__ __forceinline__ void reg_sweep_fused(const float4 (&Rr)[RPT][NV], const float* p_s, float pscale, float* ttil_s,
+template <int GT, int NV, int RPT, bool WPRE = false, class RB>
+__device__ __forceinline__ void reg_sweep_fused(const RB& Rr, const float* p_s, float pscale, float* ttil_s,
                                                 float* qs, float* red_s, double* sgrp, int ldr) {
   static_assert(RPT <= 8, "one batch of at most 8 rows per group");
   constexpr int SEG = GT < 32 ? GT : 32;
@@ -182,7 +207,7 @@ __device__ __forceinline__ void reg_sweep_fused(const float4 (&Rr)[RPT][NV], con
     float a = 0.f;
     if (i < RPT) {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) a = dot4(Rr[i < RPT ? i : 0][v], p4[v], a);
+      for (int v = 0; v < NV; ++v) a = dot4(Rr.get(i < RPT ? i : 0, v), p4[v], a);
     }
     part[i] = a;
   }
@@ -212,15 +237,15 @@ __device__ __forceinline__ void reg_sweep_fused(const float4 (&Rr)[RPT][NV], con
 #pragma unroll
   for (int i = 0; i < RPT; ++i)
 #pragma unroll
-    for (int v = 0; v < NV; ++v) axpy4(q4[v], Rr[i][v], tt[i]);
+    for (int v = 0; v < NV; ++v) axpy4(q4[v], Rr.get(i, v), tt[i]);
   store_q_partial<GT, NV>(q4, qs, g, gl, ldr, WPRE);
   __syncthreads();
 }
 
 // LOADS sweep at the start of component k:  t0 <- column k of the (already deflated) residual (S1,
 // PAPER.md:556,:1017);  q = R^T t0 (S2).  Same outputs as reg_sweep_fused.
-template <int GT, int NV, int RPT, bool WPRE = false>
-__device__ __forceinline__ void reg_sweep_loads(const float4 (&Rr)[RPT][NV], int k, float* ttil_s, float* qs, double* sgrp,
+template <int GT, int NV, int RPT, bool WPRE = false, class RB>
+__device__ __forceinline__ void reg_sweep_loads(const RB& Rr, int k, float* ttil_s, float* qs, double* sgrp,
                                                 int ldr) {
   const int tid = threadIdx.x, g = tid / GT, gl = tid - g * GT;
   const int kc = k >> 2, ke = k & 3;
@@ -231,7 +256,7 @@ __device__ __forceinline__ void reg_sweep_loads(const float4 (&Rr)[RPT][NV], int
       if (v == kv) {
 #pragma unroll
         for (int i = 0; i < RPT; ++i) {
-          const float4 x = Rr[i][v];
+          const float4 x = Rr.get(i, v);
           ttil_s[g * RPT + i] = ke == 0 ? x.x : (ke == 1 ? x.y : (ke == 2 ? x.z : x.w));
         }
       }
@@ -247,7 +272,7 @@ __device__ __forceinline__ void reg_sweep_loads(const float4 (&Rr)[RPT][NV], int
     const float t = ttil_s[g * RPT + i];
     sacc += (double)t * (double)t;
 #pragma unroll
-    for (int v = 0; v < NV; ++v) axpy4(q4[v], Rr[i][v], t);
+    for (int v = 0; v < NV; ++v) axpy4(q4[v], Rr.get(i, v), t);
   }
   if (gl == 0) sgrp[g] = sacc;
   store_q_partial<GT, NV>(q4, qs, g, gl, ldr, WPRE);
@@ -462,7 +487,7 @@ __device__ __forceinline__ void reg_gather_a(const RegParams& prm, const u64* Ax
 }
 
 // ------------------------------------------------------------------------------------ the kernel
-template <int GT, int NV, int RPT>
+template <int GT, int NV, int RPT, int RS = 0>          // RS: rows of the thread's row block kept in shared memory (RowBlock)
 __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams prm) {
   extern __shared__ __align__(16) unsigned char smem[];
   constexpr int NG = kThreads / GT;
@@ -514,13 +539,16 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
   float* Tb = prm.T + m0;
 
   // ---- R <- X: this thread's part of the CTA's row block, into registers ----
-  float4 Rr[RPT][NV];
+  RowBlock<NV, RPT, RS> Rr;
+  Rr.sm = reinterpret_cast<float4*>(smem + prm.off_rsm) + (size_t)(g * RS) * (ldr >> 2) + gl;
+  Rr.rstride = ldr >> 2;
+  Rr.vstride = GT;
 #pragma unroll
   for (int i = 0; i < RPT; ++i) {
     const int r = g * RPT + i;
 #pragma unroll
     for (int v = 0; v < NV; ++v)
-      Rr[i][v] = (r < mb) ? ld_stream4(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      Rr.set(i, v, (r < mb) ? ld_stream4(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) : make_float4(0.f, 0.f, 0.f, 0.f));
   }
   for (int i = tid; i < NG * RPT; i += kThreads) { d_s[i] = 0.f; ttil_s[i] = 0.f; }
   for (int n = tid; n < 2 * ldr; n += kThreads) p_s[n] = 0.f;
@@ -967,7 +995,11 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
       for (int i = 0; i < RPT; ++i) {
         const float dr = -d_s[g * RPT + i];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) axpy4(Rr[i][v], p4[v], dr);
+        for (int v = 0; v < NV; ++v) {
+          float4 x = Rr.get(i, v);
+          axpy4(x, p4[v], dr);
+          Rr.set(i, v, x);
+        }
       }
     }
     reg_trace(prm, tn, TR_FINAL);
@@ -980,7 +1012,7 @@ __global__ void __launch_bounds__(kThreads, 1) pca_reg_kernel(const RegParams pr
     const int r = g * RPT + i;
     if (r < mb) {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) = Rr[i][v];
+      for (int v = 0; v < NV; ++v) *reinterpret_cast<float4*>(Rb + (size_t)r * ldr + 4 * (gl + GT * v)) = Rr.get(i, v);
     }
   }
 }
@@ -1009,6 +1041,6 @@ static __global__ void __launch_bounds__(256) pca_transpose_plain_kernel(const f
 
 typedef void (*reg_kernel_t)(const RegParams);
 // defined in pca_reg_inst*.cu: the compiled (GT, RPT) variants (NV = 2), nullptr if absent
-reg_kernel_t reg_kernel_lookup(int GT, int RPT);
+reg_kernel_t reg_kernel_lookup(int GT, int RPT, int RS);
 
 }  // namespace pca

@@ -1,9 +1,9 @@
 // Instantiations of the register-resident solve kernel (pca_reg.cuh), split over several translation
-// units (-DPCA_REG_PART=0..3) so that they compile in parallel.  NV = 2 (eight columns per thread and row).
+// units (-DPCA_REG_PART=0..5) so that they compile in parallel.  NV = 2 (eight columns per thread and row).
 #include "pca_one.cuh"
 
 #ifndef PCA_REG_PART
-#error "compile with -DPCA_REG_PART=<0..3>"
+#error "compile with -DPCA_REG_PART=<0..5>"
 #endif
 
 namespace pca {
@@ -15,6 +15,9 @@ namespace pca {
 #define PCA_OV(GT, RPT) \
   if (gt == GT && rpt == RPT) return pca_one_kernel<GT, RPT>;
 #define PCA_OV3(GT) PCA_OV(GT, 2) PCA_OV(GT, 4) PCA_OV(GT, 7)
+
+#define PCA_RVS(GT) \
+  if (gt == GT) return pca_reg_kernel<GT, 2, 7, kRegSmemRows>;
 
 #if PCA_REG_PART == 0
 reg_kernel_t reg_kernel_lookup_part0(int gt, int rpt) {
@@ -39,9 +42,21 @@ reg_kernel_t reg_kernel_lookup_part2(int gt, int rpt) {
   PCA_RV3(128) PCA_RV(256, 7)
   return nullptr;
 }
-#else
+#elif PCA_REG_PART == 3
 reg_kernel_t reg_kernel_lookup_part3(int gt, int rpt) {
   PCA_RV(256, 2) PCA_RV(256, 4) PCA_RV3(512)
+  return nullptr;
+}
+// the RPT = 7 variants with kRegSmemRows rows of the row block in shared memory (fewer spills; the plan takes them when shared
+// memory is not needed for the panels)
+#elif PCA_REG_PART == 4
+reg_kernel_t reg_kernel_lookup_part4(int gt) {
+  PCA_RVS(8) PCA_RVS(16) PCA_RVS(32) PCA_RVS(64)
+  return nullptr;
+}
+#else
+reg_kernel_t reg_kernel_lookup_part5(int gt) {
+  PCA_RVS(128) PCA_RVS(256) PCA_RVS(512)
   return nullptr;
 }
 #endif
